@@ -1,0 +1,180 @@
+/*
+ * pdllm.h -- C ABI of the B200-native (sm_100a) decode-stage hot path of
+ * Prefilling-dLLM (arxiv/paper_2606_10537).
+ *
+ * Citations: "P:<line>" = /root/reference/PAPER.md line; "R<n>" = a reading of the
+ * paper listed in DESIGN.md; "S8(x)" = SURVEY.md section 8.
+ *
+ * The path (S8(a)): at every denoising step the decode-block rows attend,
+ * bidirectionally and unmasked, over
+ *     [ selected prefix KV  ||  the decode block's own KV ]
+ * where the prefix was prefilled once as N chunks of C tokens, each with a BOS
+ * token prepended, only the top-K chunks are read, each thinned to
+ * Bk kept slots by a token-keep index list (top-B retention), the selected
+ * KV sequence is cut into Split-S shards whose partial softmax results are merged
+ * by a log-sum-exp reduction.  Chunk relevance scoring and the top-K
+ * selection are part of the same path (R1).
+ *
+ * General rules for every entry point unless stated otherwise
+ *   - extern "C"; returns int: 0 = PDLLM_OK, < 0 = error (see pdllm_status).
+ *   - ENQUEUE-ONLY on the given stream: never synchronises, never allocates or
+ *     frees device memory, keeps no state between calls (TMA descriptors are
+ *     passed to kernels by value).
+ *   - "device" pointers are caller-owned device memory (e.g. a torch allocation),
+ *     16-byte aligned, dense row-major in the stated shape; inputs are read-only;
+ *     outputs are fully overwritten; buffers must stay alive until the stream has
+ *     run the enqueued work.
+ *   - Validation is host-side only (null pointer, misalignment, unsupported shape,
+ *     workspace too small): the call returns an error and enqueues nothing.
+ *     Device-side data errors (chunk id outside [0,N), keep slot outside [0,C],
+ *     unsorted keep list) are undefined behaviour.
+ *   - bf16 = IEEE bfloat16 bit patterns; O is rounded to bf16 round-to-nearest-even
+ *     from the fp32 accumulator (R11).
+ *   - GQA: query head h reads KV head h / (H / H_kv) (R4).
+ *   - scale multiplies q.k before the softmax; LSE and scores are natural logs (R5).
+ */
+#ifndef PDLLM_H_
+#define PDLLM_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* A CUDA stream handle (cudaStream_t / CUstream) passed as an opaque pointer;
+ * NULL is the legacy default stream. */
+typedef void *pdllm_stream_t;
+
+typedef enum {
+    PDLLM_OK = 0,
+    PDLLM_ERR_NULL = -1,        /* a required pointer is NULL */
+    PDLLM_ERR_ALIGN = -2,       /* a device pointer or stride is not 16-byte aligned */
+    PDLLM_ERR_SHAPE = -3,       /* a shape field is out of range (see pdllm_shape) */
+    PDLLM_ERR_WORKSPACE = -4,   /* workspace_bytes smaller than pdllm_workspace_bytes() */
+    PDLLM_ERR_UNSUPPORTED = -5, /* valid request that this build does not implement */
+    PDLLM_ERR_CUDA = -6         /* a CUDA runtime / driver call or a launch failed */
+} pdllm_status;
+
+/* Shapes shared by all calls (S8 symbols).
+ *   Cp   = C + 1 cache rows per chunk, slot 0 = the chunk's BOS (R14)
+ *   S_pre = K * Bk selected prefix rows, S_kv = S_pre + L_s                     */
+typedef struct {
+    int32_t B;      /* batch, >= 1 */
+    int32_t H;      /* query heads, H % H_kv == 0 */
+    int32_t H_kv;   /* KV heads */
+    int32_t d;      /* head dim, 64 or 128 */
+    int32_t N;      /* chunks in the cached prefix, 1..4096 */
+    int32_t C;      /* tokens per chunk (cache rows per chunk = C + 1) */
+    int32_t K;      /* chunks selected, 1 <= K <= min(N, 64) */
+    int32_t Bk;     /* kept rows per chunk incl. BOS, 1..C+1; must be C+1 when token_keep_idx == NULL */
+    int32_t L_q;    /* rows of Q used for scoring (the query window), >= 1 */
+    int32_t L;      /* rows of Q_dec / O / LSE per head, >= 1 */
+    int32_t L_s;    /* rows of K_dec / V_dec per KV head, >= 1 (R8) */
+    float   scale;  /* softmax scale; <= 0 selects 1/sqrt(d) (R5) */
+} pdllm_shape;
+
+/* ---- host-only, pure helpers (no CUDA call, usable without a GPU) ---------- */
+
+int pdllm_version(void);                       /* e.g. 100 = 0.1.0 */
+const char *pdllm_strerror(int status);        /* static string, never NULL */
+
+/* a6 (S8(a); P:189-191 fixes S = 4, NS: "chosen from N*K*C and the number of
+ * SMs"): smallest split count that gives about one wave of CTAs on num_sms SMs
+ * while leaving every split at least two 128-row KV tiles.  >= 1. */
+int32_t pdllm_auto_splits(const pdllm_shape *shape, int32_t num_sms);
+
+/* Bytes of scratch pdllm_sparse_attn / pdllm_step need for n_splits splits
+ * (n_splits == 0: the auto choice for num_sms).  0 when no scratch is needed.
+ * Returns 0 for an invalid shape. */
+size_t pdllm_workspace_bytes(const pdllm_shape *shape, int32_t n_splits, int32_t num_sms);
+
+/* Bytes of device scratch pdllm_step_host needs (staging of the per-step tensors
+ * + pdllm_workspace_bytes). */
+size_t pdllm_step_host_scratch_bytes(const pdllm_shape *shape, int32_t n_splits, int32_t num_sms);
+
+/* ---- a1: chunk-score reduction (Eq. 5; R1, R2, R3) ----------
+ * scores[b,g,n] = mean over the G*L_q rows (h in group g, i < L_q) of
+ *                 log sum_{j=0..C} exp(scale * <Q[b,h,i,:], Kcache[b,g,n,j,:]>)
+ * BOS included, keep mask not applied; higher = more relevant.
+ *   Q       device bf16, row (b,h,i) at Q + b*q_batch_stride + h*q_head_stride + i*d
+ *           (strides in elements, multiples of 8) -- lets the first L_q rows of
+ *           Q_dec [B,H,L,d] be scored in place
+ *   Kcache  device bf16 [B,H_kv,N,C+1,d]
+ *   scores  device fp32 [B,H_kv,N] (out)                                          */
+int pdllm_score_chunks(const pdllm_shape *shape, const void *Q, int64_t q_batch_stride,
+                       int64_t q_head_stride, const void *Kcache, float *scores,
+                       pdllm_stream_t stream);
+
+/* ---- a2: warp-level top-K (R6) ----------------------------------------
+ * Per (b,g): the K highest scores, ties to the lower index, NaN treated as -inf;
+ * the K chunk ids are written in ascending index order.
+ *   scores    device fp32 [B,H_kv,N];  chunk_ids  device int32 [B,H_kv,K] (out)   */
+int pdllm_select_topk(const pdllm_shape *shape, const float *scores, int32_t *chunk_ids,
+                      pdllm_stream_t stream);
+
+/* ---- a3: gather-index build (R7) ----------------------------------
+ * gather_idx[b,g,k*Bk+t] = chunk_ids[b,g,k]*(C+1) + token_keep_idx[b,g,chunk_ids[b,g,k],t]
+ * (token_keep_idx == NULL: slot t).  The attention kernel evaluates the same
+ * device function inline; this entry point exports the list.
+ *   token_keep_idx  device int32 [B,H_kv,N,Bk] ascending slots in [0,C], [..,0]==0, or NULL
+ *   gather_idx      device int32 [B,H_kv,K*Bk] (out)                              */
+int pdllm_gather_idx(const pdllm_shape *shape, const int32_t *chunk_ids,
+                     const int32_t *token_keep_idx, int32_t *gather_idx, pdllm_stream_t stream);
+
+/* ---- a4 + a5: Split-S partial attention and LSE combine (R8-R11)
+ * For every (b,h,i<L): softmax attention of Q_dec[b,h,i] over the S_kv rows
+ *   [ Kcache/Vcache rows gather_idx[b,g,:]  ||  K_dec/V_dec[b,g,:] ],  g = h/(H/H_kv),
+ * computed as n_splits partial softmax passes over contiguous ranges of those rows
+ * merged by log-sum-exp (exactly the unsplit result up to fp32 rounding).
+ *   Q_dec   device bf16 [B,H,L,d];   Kcache,Vcache device bf16 [B,H_kv,N,C+1,d]
+ *   chunk_ids device int32 [B,H_kv,K];  token_keep_idx device int32 [B,H_kv,N,Bk] or NULL
+ *   K_dec,V_dec device bf16 [B,H_kv,L_s,d]
+ *   n_splits  >= 1, or 0 = pdllm_auto_splits (capped so that no split is empty)
+ *   O       device bf16 [B,H,L,d] (out);  LSE device fp32 [B,H,L] (out)
+ *   gather_idx_out  device int32 [B,H_kv,K*Bk] (out) or NULL
+ *   workspace  device scratch of >= pdllm_workspace_bytes(shape, n_splits, num_sms) bytes
+ *              (may be NULL when that is 0)                                        */
+int pdllm_sparse_attn(const pdllm_shape *shape, const void *Q_dec, const void *Kcache,
+                      const void *Vcache, const int32_t *chunk_ids, const int32_t *token_keep_idx,
+                      const void *K_dec, const void *V_dec, int32_t n_splits,
+                      void *O, float *LSE, int32_t *gather_idx_out,
+                      void *workspace, size_t workspace_bytes, pdllm_stream_t stream);
+
+/* ---- a5 alone: LSE combine of normalised partials ---------------------
+ * LSE = log sum_s exp(lse_s);  O = sum_s exp(lse_s - LSE) * O_s;  a split with
+ * lse_s = -inf contributes nothing; all -inf gives O = 0, LSE = -inf.
+ *   O_part device fp32 [S,rows,d]; lse_part device fp32 [S,rows];
+ *   O device bf16 [rows,d] (out); LSE device fp32 [rows] (out); d in {64,128}    */
+int pdllm_lse_combine(const float *O_part, const float *lse_part, int32_t S, int64_t rows,
+                      int32_t d, void *O, float *LSE, pdllm_stream_t stream);
+
+/* ---- the per-step call: a1 -> a2 -> (a3) -> a4 -> a5 as one enqueue sequence ---
+ * Rows 0..L_q-1 of every head of Q_dec are the scoring rows (R8).
+ * scores_out [B,H_kv,N] fp32 and chunk_ids_out [B,H_kv,K] int32 are required
+ * device outputs (they carry the data between the kernels).                       */
+int pdllm_step(const pdllm_shape *shape, const void *Q_dec, const void *Kcache, const void *Vcache,
+               const int32_t *token_keep_idx, const void *K_dec, const void *V_dec, int32_t n_splits,
+               float *scores_out, int32_t *chunk_ids_out, void *O, float *LSE,
+               int32_t *gather_idx_out, void *workspace, size_t workspace_bytes,
+               pdllm_stream_t stream);
+
+/* ---- the per-step call with HOST per-step tensors ------------------------------
+ * The prefix cache and keep lists are state that the prefill left on the device
+ * ("static cache that is reused across all T denoising steps"); what
+ * changes every step is the decode block.  This call enqueues, on `stream`:
+ * H2D copies of h_Q_dec/h_K_dec/h_V_dec (host, pinned for true async) into
+ * d_scratch, pdllm_step, and D2H copies of O, LSE and chunk ids into the host
+ * outputs.  The caller synchronises the stream before reading them.
+ *   d_scratch  device scratch of >= pdllm_step_host_scratch_bytes() bytes         */
+int pdllm_step_host(const pdllm_shape *shape, const void *h_Q_dec, const void *h_K_dec,
+                    const void *h_V_dec, const void *d_Kcache, const void *d_Vcache,
+                    const int32_t *d_token_keep_idx, int32_t n_splits,
+                    void *h_O, float *h_LSE, int32_t *h_chunk_ids,
+                    void *d_scratch, size_t scratch_bytes, pdllm_stream_t stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PDLLM_H_ */
