@@ -1,0 +1,256 @@
+// pdllm_api.cu -- the C-ABI entry points of include/pdllm.h: host-side validation, shape
+// resolution, split-count choice, workspace carving and the enqueue sequences.  No arithmetic
+// of the method happens on the host.
+#include <cmath>
+#include <cstdint>
+
+#include "pdllm_internal.h"
+
+namespace pdllm {
+
+int device_num_sms() {
+    static int sms = [] {
+        int dev = 0, n = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess) return 148;
+        if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) return 148;
+        return n;
+    }();
+    return sms;
+}
+
+namespace {
+
+bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+int resolve(const pdllm_shape *sh, bool has_keep, Dims *out) {
+    if (!sh) return PDLLM_ERR_NULL;
+    if (sh->B < 1 || sh->H < 1 || sh->H_kv < 1 || sh->H % sh->H_kv != 0) return PDLLM_ERR_SHAPE;
+    if (sh->d != 64 && sh->d != 128) return PDLLM_ERR_SHAPE;
+    if (sh->N < 1 || sh->N > 4096 || sh->C < 1) return PDLLM_ERR_SHAPE;
+    if (sh->K < 1 || sh->K > sh->N || sh->K > 64) return PDLLM_ERR_SHAPE;
+    if (sh->Bk < 1 || sh->Bk > sh->C + 1) return PDLLM_ERR_SHAPE;
+    if (!has_keep && sh->Bk != sh->C + 1) return PDLLM_ERR_SHAPE;
+    if (sh->L_q < 1 || sh->L < 1 || sh->L_s < 1) return PDLLM_ERR_SHAPE;
+    const int64_t cache_rows = (int64_t)sh->B * sh->H_kv * sh->N * (sh->C + 1);
+    if (cache_rows >= (1ll << 31)) return PDLLM_ERR_SHAPE;
+    if ((int64_t)sh->K * sh->Bk + sh->L_s >= (1ll << 30)) return PDLLM_ERR_SHAPE;
+    if ((int64_t)sh->B * sh->H_kv > 65535) return PDLLM_ERR_SHAPE;
+    Dims d;
+    d.B = sh->B; d.H = sh->H; d.H_kv = sh->H_kv; d.G = sh->H / sh->H_kv; d.d = sh->d;
+    d.N = sh->N; d.C = sh->C; d.Cp = sh->C + 1; d.K = sh->K; d.Bk = sh->Bk;
+    d.L_q = sh->L_q; d.L = sh->L; d.L_s = sh->L_s;
+    d.S_pre = sh->K * sh->Bk; d.S_kv = d.S_pre + sh->L_s;
+    d.rows_g = d.G * sh->L;
+    d.scale = sh->scale > 0.f ? sh->scale : 1.0f / std::sqrt((float)sh->d);
+    *out = d;
+    return PDLLM_OK;
+}
+
+int kv_tiles(const Dims &d) { return (d.S_kv + kTileN - 1) / kTileN; }
+int m_tiles(const Dims &d) { return d.B * d.H_kv * ((d.rows_g + kTileM - 1) / kTileM); }
+
+// a6: smallest S with about one wave of CTAs (2 resident per SM) and >= 2 KV tiles per split.
+int auto_splits(const Dims &d, int num_sms) {
+    const int T = kv_tiles(d), M = m_tiles(d);
+    const int slots = 2 * (num_sms > 0 ? num_sms : 148);
+    int S = 1;
+    while (M * S < slots && T / (S + 1) >= 2) ++S;
+    return S;
+}
+
+int effective_splits(const Dims &d, int n_splits, int num_sms) {
+    int S = n_splits == 0 ? auto_splits(d, num_sms) : n_splits;
+    const int T = kv_tiles(d);
+    return S > T ? T : S;       // no empty split (R10)
+}
+
+size_t workspace_for(const Dims &d, int S) {
+    if (S <= 1) return 0;
+    const size_t rows = (size_t)d.B * d.H * d.L;
+    return align_up((size_t)S * rows * d.d * sizeof(float), 256) + align_up((size_t)S * rows * sizeof(float), 256);
+}
+
+struct HostScratch {
+    size_t q, kd, vd, scores, ids, o, lse, ws, total;
+};
+HostScratch host_scratch(const Dims &d, int S) {
+    HostScratch h;
+    size_t off = 0;
+    auto take = [&](size_t bytes) { size_t o = off; off += align_up(bytes, 256); return o; };
+    h.q = take((size_t)d.B * d.H * d.L * d.d * 2);
+    h.kd = take((size_t)d.B * d.H_kv * d.L_s * d.d * 2);
+    h.vd = take((size_t)d.B * d.H_kv * d.L_s * d.d * 2);
+    h.scores = take((size_t)d.B * d.H_kv * d.N * 4);
+    h.ids = take((size_t)d.B * d.H_kv * d.K * 4);
+    h.o = take((size_t)d.B * d.H * d.L * d.d * 2);
+    h.lse = take((size_t)d.B * d.H * d.L * 4);
+    h.ws = off;
+    off += workspace_for(d, S);
+    h.total = off;
+    return h;
+}
+
+int cuda_rc(cudaError_t e) { return e == cudaSuccess ? PDLLM_OK : PDLLM_ERR_CUDA; }
+
+}  // namespace
+}  // namespace pdllm
+
+using namespace pdllm;
+
+extern "C" {
+
+int pdllm_version(void) { return 100; }
+
+const char *pdllm_strerror(int status) {
+    switch (status) {
+        case PDLLM_OK: return "ok";
+        case PDLLM_ERR_NULL: return "a required pointer is NULL";
+        case PDLLM_ERR_ALIGN: return "a device pointer or stride is not 16-byte aligned";
+        case PDLLM_ERR_SHAPE: return "a shape field is out of range";
+        case PDLLM_ERR_WORKSPACE: return "workspace too small";
+        case PDLLM_ERR_UNSUPPORTED: return "unsupported request";
+        case PDLLM_ERR_CUDA: return "CUDA call or launch failed";
+        default: return "unknown pdllm status";
+    }
+}
+
+int32_t pdllm_auto_splits(const pdllm_shape *shape, int32_t num_sms) {
+    Dims d;
+    if (resolve(shape, shape && shape->Bk != shape->C + 1, &d) != PDLLM_OK) return 1;
+    return effective_splits(d, 0, num_sms);
+}
+
+size_t pdllm_workspace_bytes(const pdllm_shape *shape, int32_t n_splits, int32_t num_sms) {
+    Dims d;
+    if (n_splits < 0 || resolve(shape, shape && shape->Bk != shape->C + 1, &d) != PDLLM_OK) return 0;
+    return workspace_for(d, effective_splits(d, n_splits, num_sms));
+}
+
+size_t pdllm_step_host_scratch_bytes(const pdllm_shape *shape, int32_t n_splits, int32_t num_sms) {
+    Dims d;
+    if (n_splits < 0 || resolve(shape, shape && shape->Bk != shape->C + 1, &d) != PDLLM_OK) return 0;
+    return host_scratch(d, effective_splits(d, n_splits, num_sms)).total;
+}
+
+int pdllm_score_chunks(const pdllm_shape *shape, const void *Q, int64_t q_batch_stride, int64_t q_head_stride,
+                       const void *Kcache, float *scores, pdllm_stream_t stream) {
+    if (!shape || !Q || !Kcache || !scores) return PDLLM_ERR_NULL;
+    Dims d;
+    // scoring never reads the keep list (R3): Bk is not constrained here
+    pdllm_shape sh = *shape;
+    sh.Bk = sh.C + 1;
+    if (int rc = resolve(&sh, false, &d)) return rc;
+    if (!aligned16(Q) || !aligned16(Kcache) || !aligned16(scores)) return PDLLM_ERR_ALIGN;
+    if ((q_batch_stride & 7) || (q_head_stride & 7) || q_head_stride < (int64_t)d.L_q * d.d) return PDLLM_ERR_ALIGN;
+    return cuda_rc(launch_score(d, Q, q_batch_stride, q_head_stride, Kcache, scores, static_cast<cudaStream_t>(stream)));
+}
+
+int pdllm_select_topk(const pdllm_shape *shape, const float *scores, int32_t *chunk_ids, pdllm_stream_t stream) {
+    if (!shape || !scores || !chunk_ids) return PDLLM_ERR_NULL;
+    Dims d;
+    pdllm_shape sh = *shape;
+    sh.Bk = sh.C + 1;
+    if (int rc = resolve(&sh, false, &d)) return rc;
+    return cuda_rc(launch_topk(d, scores, chunk_ids, static_cast<cudaStream_t>(stream)));
+}
+
+int pdllm_gather_idx(const pdllm_shape *shape, const int32_t *chunk_ids, const int32_t *token_keep_idx,
+                     int32_t *gather_idx, pdllm_stream_t stream) {
+    if (!shape || !chunk_ids || !gather_idx) return PDLLM_ERR_NULL;
+    Dims d;
+    if (int rc = resolve(shape, token_keep_idx != nullptr, &d)) return rc;
+    return cuda_rc(launch_gather_idx(d, chunk_ids, token_keep_idx, gather_idx, static_cast<cudaStream_t>(stream)));
+}
+
+int pdllm_lse_combine(const float *O_part, const float *lse_part, int32_t S, int64_t rows, int32_t d, void *O, float *LSE,
+                      pdllm_stream_t stream) {
+    if (!O_part || !lse_part || !O || !LSE) return PDLLM_ERR_NULL;
+    if (S < 1 || rows < 1 || (d != 64 && d != 128)) return PDLLM_ERR_SHAPE;
+    if (!aligned16(O_part) || !aligned16(O)) return PDLLM_ERR_ALIGN;
+    return cuda_rc(launch_combine(O_part, lse_part, S, rows, d, O, LSE, static_cast<cudaStream_t>(stream)));
+}
+
+int pdllm_sparse_attn(const pdllm_shape *shape, const void *Q_dec, const void *Kcache, const void *Vcache,
+                      const int32_t *chunk_ids, const int32_t *token_keep_idx, const void *K_dec, const void *V_dec,
+                      int32_t n_splits, void *O, float *LSE, int32_t *gather_idx_out, void *workspace,
+                      size_t workspace_bytes, pdllm_stream_t stream) {
+    if (!shape || !Q_dec || !Kcache || !Vcache || !chunk_ids || !K_dec || !V_dec || !O || !LSE) return PDLLM_ERR_NULL;
+    if (n_splits < 0) return PDLLM_ERR_SHAPE;
+    Dims d;
+    if (int rc = resolve(shape, token_keep_idx != nullptr, &d)) return rc;
+    if (!aligned16(Q_dec) || !aligned16(Kcache) || !aligned16(Vcache) || !aligned16(K_dec) || !aligned16(V_dec) ||
+        !aligned16(O) || !aligned16(workspace))
+        return PDLLM_ERR_ALIGN;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const int S = effective_splits(d, n_splits, device_num_sms());
+    const size_t need = workspace_for(d, S);
+    if (need > 0 && (!workspace || workspace_bytes < need)) return PDLLM_ERR_WORKSPACE;
+    if (gather_idx_out)
+        if (int rc = cuda_rc(launch_gather_idx(d, chunk_ids, token_keep_idx, gather_idx_out, st))) return rc;
+    const size_t rows = (size_t)d.B * d.H * d.L;
+    float *O_part = nullptr, *lse_part = nullptr;
+    if (S > 1) {
+        O_part = static_cast<float *>(workspace);
+        lse_part = reinterpret_cast<float *>(static_cast<char *>(workspace) + align_up((size_t)S * rows * d.d * sizeof(float), 256));
+    }
+    if (int rc = cuda_rc(launch_attn(d, Q_dec, Kcache, Vcache, chunk_ids, token_keep_idx, K_dec, V_dec, S, O, LSE, O_part,
+                                     lse_part, st)))
+        return rc;
+    if (S > 1) return cuda_rc(launch_combine(O_part, lse_part, S, (int64_t)rows, d.d, O, LSE, st));
+    return PDLLM_OK;
+}
+
+int pdllm_step(const pdllm_shape *shape, const void *Q_dec, const void *Kcache, const void *Vcache,
+               const int32_t *token_keep_idx, const void *K_dec, const void *V_dec, int32_t n_splits, float *scores_out,
+               int32_t *chunk_ids_out, void *O, float *LSE, int32_t *gather_idx_out, void *workspace,
+               size_t workspace_bytes, pdllm_stream_t stream) {
+    if (!shape || !scores_out || !chunk_ids_out) return PDLLM_ERR_NULL;
+    if (shape->L_q > shape->L) return PDLLM_ERR_SHAPE;
+    // validate the attention arguments before anything is enqueued
+    if (!Q_dec || !Kcache || !Vcache || !K_dec || !V_dec || !O || !LSE) return PDLLM_ERR_NULL;
+    Dims d;
+    if (int rc = resolve(shape, token_keep_idx != nullptr, &d)) return rc;
+    if (n_splits < 0) return PDLLM_ERR_SHAPE;
+    const size_t need = workspace_for(d, effective_splits(d, n_splits, device_num_sms()));
+    if (need > 0 && (!workspace || workspace_bytes < need)) return PDLLM_ERR_WORKSPACE;
+    if (int rc = pdllm_score_chunks(shape, Q_dec, (int64_t)d.H * d.L * d.d, (int64_t)d.L * d.d, Kcache, scores_out, stream))
+        return rc;
+    if (int rc = pdllm_select_topk(shape, scores_out, chunk_ids_out, stream)) return rc;
+    return pdllm_sparse_attn(shape, Q_dec, Kcache, Vcache, chunk_ids_out, token_keep_idx, K_dec, V_dec, n_splits, O, LSE,
+                             gather_idx_out, workspace, workspace_bytes, stream);
+}
+
+int pdllm_step_host(const pdllm_shape *shape, const void *h_Q_dec, const void *h_K_dec, const void *h_V_dec,
+                    const void *d_Kcache, const void *d_Vcache, const int32_t *d_token_keep_idx, int32_t n_splits,
+                    void *h_O, float *h_LSE, int32_t *h_chunk_ids, void *d_scratch, size_t scratch_bytes,
+                    pdllm_stream_t stream) {
+    if (!shape || !h_Q_dec || !h_K_dec || !h_V_dec || !d_Kcache || !d_Vcache || !h_O || !h_LSE || !h_chunk_ids || !d_scratch)
+        return PDLLM_ERR_NULL;
+    if (n_splits < 0) return PDLLM_ERR_SHAPE;
+    Dims d;
+    if (int rc = resolve(shape, d_token_keep_idx != nullptr, &d)) return rc;
+    if (!aligned16(d_scratch)) return PDLLM_ERR_ALIGN;
+    const int S = effective_splits(d, n_splits, device_num_sms());
+    const HostScratch h = host_scratch(d, S);
+    if (scratch_bytes < h.total) return PDLLM_ERR_WORKSPACE;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    char *base = static_cast<char *>(d_scratch);
+    const size_t qb = (size_t)d.B * d.H * d.L * d.d * 2, kb = (size_t)d.B * d.H_kv * d.L_s * d.d * 2;
+    if (cudaMemcpyAsync(base + h.q, h_Q_dec, qb, cudaMemcpyHostToDevice, st) != cudaSuccess) return PDLLM_ERR_CUDA;
+    if (cudaMemcpyAsync(base + h.kd, h_K_dec, kb, cudaMemcpyHostToDevice, st) != cudaSuccess) return PDLLM_ERR_CUDA;
+    if (cudaMemcpyAsync(base + h.vd, h_V_dec, kb, cudaMemcpyHostToDevice, st) != cudaSuccess) return PDLLM_ERR_CUDA;
+    if (int rc = pdllm_step(shape, base + h.q, d_Kcache, d_Vcache, d_token_keep_idx, base + h.kd, base + h.vd, n_splits,
+                            reinterpret_cast<float *>(base + h.scores), reinterpret_cast<int32_t *>(base + h.ids),
+                            base + h.o, reinterpret_cast<float *>(base + h.lse), nullptr, base + h.ws,
+                            h.total - h.ws, stream))
+        return rc;
+    if (cudaMemcpyAsync(h_O, base + h.o, qb, cudaMemcpyDeviceToHost, st) != cudaSuccess) return PDLLM_ERR_CUDA;
+    if (cudaMemcpyAsync(h_LSE, base + h.lse, (size_t)d.B * d.H * d.L * 4, cudaMemcpyDeviceToHost, st) != cudaSuccess)
+        return PDLLM_ERR_CUDA;
+    if (cudaMemcpyAsync(h_chunk_ids, base + h.ids, (size_t)d.B * d.H_kv * d.K * 4, cudaMemcpyDeviceToHost, st) != cudaSuccess)
+        return PDLLM_ERR_CUDA;
+    return PDLLM_OK;
+}
+
+}  // extern "C"

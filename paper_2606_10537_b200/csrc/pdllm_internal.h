@@ -1,0 +1,43 @@
+// pdllm_internal.h -- declarations shared by the translation units of libpdllm.so (not installed).
+#pragma once
+#include <cuda_runtime.h>
+#include <cstddef>
+#include <cstdint>
+
+#include "../../include/pdllm.h"
+
+namespace pdllm {
+
+// pdllm_shape with the derived sizes of SURVEY 8 resolved once on the host.
+struct Dims {
+    int B, H, H_kv, G, d;
+    int N, C, Cp, K, Bk;
+    int L_q, L, L_s;
+    int S_pre, S_kv;      // K*Bk, K*Bk + L_s
+    int rows_g;           // G*L: rows of Q_dec that share one KV head (contiguous in [B,H,L,d])
+    float scale;
+};
+
+constexpr int kTileM = 128;   // query rows per CTA tile (UMMA M)
+constexpr int kTileN = 128;   // virtual KV rows per tile
+
+// ---- a2
+cudaError_t launch_topk(const Dims &s, const float *scores, int32_t *chunk_ids, cudaStream_t st);
+// ---- a3
+cudaError_t launch_gather_idx(const Dims &s, const int32_t *chunk_ids, const int32_t *keep, int32_t *gather_idx,
+                              cudaStream_t st);
+// ---- a5
+cudaError_t launch_combine(const float *O_part, const float *lse_part, int S, int64_t rows, int d, void *O, float *LSE,
+                           cudaStream_t st);
+// ---- a1: scores[b,g,n]; `partial` is scratch of score_scratch_bytes()
+size_t score_scratch_bytes(const Dims &s);
+cudaError_t launch_score(const Dims &s, const void *Q, int64_t q_batch_stride, int64_t q_head_stride, const void *Kcache,
+                         float *scores, cudaStream_t st);
+// ---- a3+a4 (+a5 when n_splits > 1)
+cudaError_t launch_attn(const Dims &s, const void *Q_dec, const void *Kcache, const void *Vcache, const int32_t *chunk_ids,
+                        const int32_t *keep, const void *K_dec, const void *V_dec, int n_splits, void *O, float *LSE,
+                        float *O_part, float *lse_part, cudaStream_t st);
+
+int device_num_sms();
+
+}  // namespace pdllm

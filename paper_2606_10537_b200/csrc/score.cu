@@ -1,0 +1,290 @@
+// score.cu -- a1: chunk-score reduction (Eq. 5; readings R1-R3), tcgen05 / TMEM / TMA.
+//
+//   scores[b,g,n] = mean over the G*L_q scoring rows of  log sum_{j<=C} exp(scale * q . Kcache[b,g,n,j])
+//
+// The kernel streams every cached K row exactly once (HBM-bound at MHA shapes).  One CTA owns a
+// 128-row tile of the scoring rows and a run of consecutive chunks of one (b,g); each chunk is
+// cut into 128-row K tiles (the tail tile is shortened to a multiple of 16 rows) that one thread
+// fetches with TMA into a ring of 128B-swizzled stages; one thread issues S = Q K^T (tcgen05.mma)
+// into one of two TMEM accumulators; the 128 softmax threads (thread = row) fold the tile into the
+// running (max, sum) of the current chunk and, at the chunk's last tile, reduce log-masses over rows.
+#include <cuda.h>
+
+#include "pdllm_internal.h"
+#include "ptx.cuh"
+
+namespace pdllm {
+
+namespace {
+
+constexpr int kScoreThreads = 192;        // 4 softmax warps + TMA warp + MMA warp
+constexpr int kMaxChunksPerCta = 64;
+
+struct ScoreParams {
+    const uint16_t *Q;
+    int64_t q_batch_stride, q_head_stride;
+    float *scores;
+    int H_kv, G, N, Cp, L_q, rows;        // rows = G * L_q
+    int m_tiles, n_groups, cpc;           // chunks per CTA
+    float c2, inv_rows;
+    int use_atomic, evict_first;
+};
+
+template <int D>
+struct ScoreCfg {
+    static constexpr int kPanels = D / 64;
+    static constexpr uint32_t kPanelBytes = 128 * 128;
+    static constexpr uint32_t kTileBytes = kPanels * kPanelBytes;
+    static constexpr int kStages = (D == 128) ? 2 : 4;
+    static constexpr size_t kSmem = 1024 + (size_t)(1 + kStages) * kTileBytes;
+};
+
+template <int D>
+__global__ void __launch_bounds__(kScoreThreads, 2)
+score_kernel(const ScoreParams p, const __grid_constant__ CUtensorMap tmap128, const __grid_constant__ CUtensorMap tmap16) {
+    using Cfg = ScoreCfg<D>;
+    constexpr int ST = Cfg::kStages;
+    constexpr int kChunksPerRow = D / 8;
+
+    extern __shared__ uint8_t smem_raw[];
+    const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+    const uint32_t sQ = smem_base;
+    auto sK = [&](int stage) { return smem_base + Cfg::kTileBytes * (uint32_t)(1 + stage); };
+
+    __shared__ uint64_t bars[2 * ST + 4];   // k_full[ST], k_free[ST], s_ready[2], s_free[2]
+    __shared__ uint32_t tmem_slot;
+    __shared__ float s_acc[kMaxChunksPerCta * 4];
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int group = blockIdx.x / p.m_tiles, mt = blockIdx.x % p.m_tiles, bg = blockIdx.y;
+    const int b = bg / p.H_kv, g = bg % p.H_kv;
+    const int n0 = group * p.cpc, n1 = min(p.N, n0 + p.cpc);
+    const int tiles_per_chunk = (p.Cp + kTileN - 1) / kTileN;
+
+    const uint32_t bar0 = smem_u32(&bars[0]);
+    auto k_full = [&](int s) { return bar0 + 8u * s; };
+    auto k_free = [&](int s) { return bar0 + 8u * (ST + s); };
+    auto s_ready = [&](int i) { return bar0 + 8u * (2 * ST + i); };
+    auto s_free = [&](int i) { return bar0 + 8u * (2 * ST + 2 + i); };
+
+    if (tid == 0) {
+        for (int s = 0; s < ST; ++s) { mbar_init(k_full(s), 1); mbar_init(k_free(s), 1); }
+        for (int i = 0; i < 2; ++i) { mbar_init(s_ready(i), 1); mbar_init(s_free(i), 128); }
+        fence_mbar_init();
+        tma_prefetch_desc(&tmap128);
+        tma_prefetch_desc(&tmap16);
+    }
+    if (warp == 5) {
+        tmem_alloc(smem_u32(&tmem_slot), 256);
+        tmem_relinquish();
+    }
+    // Q tile (scoring rows mt*128.. of group g; row m -> head g*G + m / L_q, position m % L_q)
+    for (int i = tid; i < kTileM * kChunksPerRow; i += kScoreThreads) {
+        const int r = i / kChunksPerRow, c = i % kChunksPerRow;
+        const int m = mt * kTileM + r;
+        const bool ok = m < p.rows;
+        const int hh = ok ? m / p.L_q : 0, qi = ok ? m % p.L_q : 0;
+        const uint16_t *src = p.Q + (int64_t)b * p.q_batch_stride + (int64_t)(g * p.G + hh) * p.q_head_stride +
+                              (int64_t)qi * D + c * 8;
+        cp_async16_zfill(sQ + (uint32_t)(c >> 3) * Cfg::kPanelBytes + sw128_off(r, c & 7), src, ok ? 16u : 0u);
+    }
+    cp_async_commit();
+    cp_async_wait<0>();
+    fence_proxy_async_smem();
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem = tmem_slot;
+
+    if (warp == 4) {
+        // =============================== TMA producer ===============================
+        if (lane == 0) {
+            const uint64_t policy = l2_policy_evict_first();
+            int q = 0;
+            for (int n = n0; n < n1; ++n) {
+                const int64_t row0 = ((int64_t)bg * p.N + n) * p.Cp;
+                for (int tt = 0; tt < tiles_per_chunk; ++tt, ++q) {
+                    const int stage = q % ST;
+                    const int valid = min(kTileN, p.Cp - tt * kTileN);
+                    const bool small = valid <= 16;
+                    mbar_wait(k_free(stage), ((q / ST) & 1) ^ 1);
+                    mbar_arrive_expect_tx(k_full(stage), (uint32_t)(small ? 16 : 128) * D * 2);
+                    const CUtensorMap *tm = small ? &tmap16 : &tmap128;
+                    const int32_t row = (int32_t)(row0 + (int64_t)tt * kTileN);
+#pragma unroll
+                    for (int pn = 0; pn < Cfg::kPanels; ++pn) {
+                        if (p.evict_first)
+                            tma_load_2d_hint(sK(stage) + pn * Cfg::kPanelBytes, tm, pn * 64, row, k_full(stage), policy);
+                        else
+                            tma_load_2d(sK(stage) + pn * Cfg::kPanelBytes, tm, pn * 64, row, k_full(stage));
+                    }
+                }
+            }
+        }
+        __syncwarp();
+    } else if (warp == 5) {
+        // =============================== MMA issuer ===============================
+        if (lane == 0) {
+            int q = 0;
+            for (int n = n0; n < n1; ++n) {
+                for (int tt = 0; tt < tiles_per_chunk; ++tt, ++q) {
+                    const int stage = q % ST, buf = q & 1;
+                    const int valid = min(kTileN, p.Cp - tt * kTileN);
+                    const uint32_t n_mma = (uint32_t)(valid + 15) & ~15u;
+                    mbar_wait(k_full(stage), (q / ST) & 1);
+                    mbar_wait(s_free(buf), ((q >> 1) & 1) ^ 1);
+                    tc_fence_after();
+                    const uint32_t idesc = umma_idesc_bf16(kTileM, n_mma, 0, 0);
+#pragma unroll
+                    for (int ks = 0; ks < D / 16; ++ks) {
+                        const uint32_t off = (uint32_t)(ks >> 2) * Cfg::kPanelBytes + (uint32_t)(ks & 3) * 32u;
+                        umma_ss(tmem + 128u * buf, umma_desc_sw128(sQ + off, 16, 1024),
+                                umma_desc_sw128(sK(stage) + off, 16, 1024), idesc, ks > 0);
+                    }
+                    umma_commit(s_ready(buf));
+                    umma_commit(k_free(stage));
+                }
+            }
+        }
+        __syncwarp();
+    } else {
+        // =============================== softmax (thread = row) ===============================
+        const uint32_t lane_base = (uint32_t)(warp * 32) << 16;
+        const bool row_ok = mt * kTileM + tid < p.rows;
+        int q = 0;
+        for (int n = n0; n < n1; ++n) {
+            float m_run = -INFINITY, l = 0.f;
+            for (int tt = 0; tt < tiles_per_chunk; ++tt, ++q) {
+                const int buf = q & 1;
+                const int valid = min(kTileN, p.Cp - tt * kTileN);
+                const int nchunks = (((valid + 15) & ~15) + 31) >> 5;
+                const uint32_t tS = tmem + 128u * buf + lane_base;
+                mbar_wait(s_ready(buf), (q >> 1) & 1);
+                tc_fence_after();
+                for (int ch = 0; ch < nchunks; ++ch) {
+                    uint32_t v[32];
+                    tmem_ld32(tS + 32u * ch, v);
+                    tmem_wait_ld();
+                    if (ch == nchunks - 1) {          // accumulator buffer is free once it is in registers
+                        tc_fence_before();
+                        mbar_arrive(s_free(buf));
+                    }
+                    const int nv = valid - ch * 32;   // valid columns in this 32-column chunk (may exceed 32)
+                    float cmax = -INFINITY;
+                    if (nv >= 32) {
+#pragma unroll
+                        for (int e = 0; e < 32; ++e) cmax = fmaxf(cmax, __uint_as_float(v[e]));
+                    } else {
+#pragma unroll
+                        for (int e = 0; e < 32; ++e)
+                            if (e < nv) cmax = fmaxf(cmax, __uint_as_float(v[e]));
+                    }
+                    const float m_new = fmaxf(m_run, cmax * p.c2);
+                    float sum = 0.f;
+                    if (nv >= 32) {
+#pragma unroll
+                        for (int e = 0; e < 32; ++e) sum += ex2_approx(fmaf(__uint_as_float(v[e]), p.c2, -m_new));
+                    } else {
+#pragma unroll
+                        for (int e = 0; e < 32; ++e)
+                            if (e < nv) sum += ex2_approx(fmaf(__uint_as_float(v[e]), p.c2, -m_new));
+                    }
+                    l = l * ex2_approx(m_run - m_new) + sum;
+                    m_run = m_new;
+                }
+            }
+            // chunk n finished: log-mass of this row, summed over the tile's rows (fixed order)
+            float ell = row_ok ? (m_run + lg2_approx(l)) * 0.6931471805599453f : 0.f;
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) ell += __shfl_xor_sync(0xffffffffu, ell, o);
+            if (lane == 0) s_acc[(n - n0) * 4 + warp] = ell;
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 5) tmem_dealloc(tmem, 256);
+    if (tid < n1 - n0) {
+        const float tot = ((s_acc[tid * 4 + 0] + s_acc[tid * 4 + 1]) + (s_acc[tid * 4 + 2] + s_acc[tid * 4 + 3])) * p.inv_rows;
+        float *dst = p.scores + (int64_t)bg * p.N + n0 + tid;
+        if (p.use_atomic) atomicAdd(dst, tot);
+        else *dst = tot;
+    }
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn encode_tiled_fn() {
+    static EncodeTiledFn fn = [] {
+        void *f = nullptr;
+        cudaDriverEntryPointQueryResult qr;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &f, cudaEnableDefault, &qr) != cudaSuccess ||
+            qr != cudaDriverEntryPointSuccess)
+            f = nullptr;
+        return reinterpret_cast<EncodeTiledFn>(f);
+    }();
+    return fn;
+}
+
+// bf16 [rows, d] row-major, box = [box_rows, 64 columns], 128-byte swizzle, OOB rows read as zero.
+bool make_rows_tmap(CUtensorMap *tm, const void *base, uint64_t rows, int d, int box_rows) {
+    EncodeTiledFn fn = encode_tiled_fn();
+    if (!fn) return false;
+    cuuint64_t dims[2] = {(cuuint64_t)d, rows};
+    cuuint64_t strides[1] = {(cuuint64_t)d * 2};
+    cuuint32_t box[2] = {64, (cuuint32_t)box_rows};
+    cuuint32_t es[2] = {1, 1};
+    return fn(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void *>(base), dims, strides, box, es,
+              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+template <int D>
+cudaError_t launch_score_d(const ScoreParams &p, const CUtensorMap &t128, const CUtensorMap &t16, int BG, cudaStream_t st) {
+    using Cfg = ScoreCfg<D>;
+    cudaError_t e = cudaFuncSetAttribute(score_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::kSmem);
+    if (e != cudaSuccess) return e;
+    dim3 grid((unsigned)(p.n_groups * p.m_tiles), (unsigned)BG, 1);
+    score_kernel<D><<<grid, kScoreThreads, Cfg::kSmem, st>>>(p, t128, t16);
+    return cudaGetLastError();
+}
+
+}  // namespace
+
+cudaError_t launch_score(const Dims &s, const void *Q, int64_t q_batch_stride, int64_t q_head_stride, const void *Kcache,
+                         float *scores, cudaStream_t st) {
+    ScoreParams p;
+    p.Q = static_cast<const uint16_t *>(Q);
+    p.q_batch_stride = q_batch_stride;
+    p.q_head_stride = q_head_stride;
+    p.scores = scores;
+    p.H_kv = s.H_kv; p.G = s.G; p.N = s.N; p.Cp = s.Cp; p.L_q = s.L_q;
+    p.rows = s.G * s.L_q;
+    p.m_tiles = (p.rows + kTileM - 1) / kTileM;
+    const int BG = s.B * s.H_kv;
+    // chunks per CTA: about six waves of (2 CTAs x SMs) work items, so the tail wave stays small
+    const int64_t units = (int64_t)BG * s.N * p.m_tiles;
+    const int64_t slots = 2ll * device_num_sms();
+    int cpc = (int)((units + slots * 6 - 1) / (slots * 6));
+    cpc = cpc < 1 ? 1 : (cpc > kMaxChunksPerCta ? kMaxChunksPerCta : cpc);
+    if (cpc > s.N) cpc = s.N;
+    p.cpc = cpc;
+    p.n_groups = (s.N + cpc - 1) / cpc;
+    p.c2 = s.scale * 1.4426950408889634f;
+    p.inv_rows = 1.0f / (float)p.rows;
+    p.use_atomic = p.m_tiles > 1;
+    p.evict_first = p.m_tiles == 1;
+
+    CUtensorMap t128, t16;
+    const uint64_t rows = (uint64_t)BG * s.N * s.Cp;
+    if (!make_rows_tmap(&t128, Kcache, rows, s.d, 128) || !make_rows_tmap(&t16, Kcache, rows, s.d, 16))
+        return cudaErrorInvalidValue;
+    if (p.use_atomic) {
+        cudaError_t e = cudaMemsetAsync(scores, 0, sizeof(float) * (size_t)BG * s.N, st);
+        if (e != cudaSuccess) return e;
+    }
+    return s.d == 128 ? launch_score_d<128>(p, t128, t16, BG, st) : launch_score_d<64>(p, t128, t16, BG, st);
+}
+
+}  // namespace pdllm

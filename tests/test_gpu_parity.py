@@ -1,0 +1,242 @@
+"""GPU-vs-oracle parity through the C ABI (include/pdllm.h), element by element on the same seeded
+inputs.  Bars (SURVEY 8(c) R12 / BASELINE.json north_star): chunk ids and gather indices bit-exact;
+O within 2e-2 + 1e-2|ref| per element and max|d|/max|ref| <= 1e-2; LSE and scores within 1e-3.
+"""
+import numpy as np
+import pytest
+import torch
+
+from oracle import oracle
+from paper_2606_10537_b200 import workloads as W
+
+from gpu_util import (LSE_ABS, SCORE_ABS, check_close, check_exact, check_O, dev_bf16, dev_f32, dev_i32,
+                      shape_of, to_device)
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_2606_10537_b200 import binding
+    binding.lib()
+    return binding
+
+
+def _inputs(name, **kw):
+    w = W.CONFIGS[name]
+    if kw:
+        w = W.small_variant(w, **kw)
+    return w, W.make_inputs(w)
+
+
+# --------------------------------------------------------------------------- a2 top-K
+@pytest.mark.parametrize("rows,N,K", [(4, 8, 2), (32, 16, 4), (128, 64, 8), (5, 33, 33), (3, 1, 1), (7, 100, 1),
+                                      (9, 513, 16), (2, 4096, 64), (6, 130, 64)])
+def test_topk_random(B, rows, N, K):
+    r = np.random.default_rng(rows * 1000 + N + K)
+    s = r.standard_normal((1, rows, N)).astype(np.float32)
+    shape = B.Shape(1, rows, rows, 128, N, 512, K, 513, 1, 1, 1)
+    got = B.select_topk(shape, dev_f32(s))
+    check_exact(got, oracle.topk(s, K))
+
+
+def test_topk_ties_nan_inf(B):
+    N, K = 40, 6
+    s = np.zeros((1, 6, N), np.float32)
+    s[0, 0] = 1.0                                   # all equal: lowest indices win
+    s[0, 1, ::3] = 2.0                              # many ties above a floor
+    s[0, 2] = np.nan                                # all NaN == all -inf
+    s[0, 3] = -np.inf; s[0, 3, [7, 30]] = 0.5       # fewer finite values than K
+    s[0, 4] = np.arange(N)[::-1]; s[0, 4, 5] = np.nan; s[0, 4, 0] = np.inf
+    s[0, 5] = np.tile([3.0, 1.0], N // 2)
+    shape = B.Shape(1, 6, 6, 128, N, 512, K, 513, 1, 1, 1)
+    check_exact(B.select_topk(shape, dev_f32(s)), oracle.topk(s, K))
+
+
+# --------------------------------------------------------------------------- a3 gather indices
+@pytest.mark.parametrize("name", ["tiny", "sparse32k"])
+def test_gather_idx(B, name):
+    w = W.CONFIGS[name]
+    keep, ids = W.make_keep(w), W.make_planted(w)
+    shape = B.Shape.of(w)
+    got = B.gather_idx(shape, dev_i32(ids), dev_i32(keep))
+    check_exact(got, oracle.gather_idx(ids, keep, w.N, w.C), "gather_idx")
+
+
+def test_gather_idx_no_keep(B):
+    w = W.CONFIGS["llada8k"]
+    ids = W.make_planted(w)
+    got = B.gather_idx(B.Shape.of(w), dev_i32(ids), None)
+    check_exact(got, oracle.gather_idx(ids, None, w.N, w.C), "gather_idx")
+
+
+# --------------------------------------------------------------------------- a5 combine
+@pytest.mark.parametrize("S,rows,d", [(1, 37, 128), (2, 300, 128), (4, 48, 64), (7, 1000, 128), (64, 129, 64)])
+def test_lse_combine(B, S, rows, d):
+    r = np.random.default_rng(S * 7 + rows)
+    Op = r.standard_normal((S, rows, d)).astype(np.float32)
+    lp = (3.0 * r.standard_normal((S, rows))).astype(np.float32)
+    if S > 1:
+        lp[0, ::5] = -np.inf                         # an empty split for some rows
+        lp[:, 3] = -np.inf                           # a row with nothing at all
+        Op[:, 3] = 0.0
+    O, LSE = B.lse_combine(dev_f32(Op), dev_f32(lp))
+    O_ref, LSE_ref = oracle.lse_combine(Op, lp)
+    check_O(O, O_ref, what="combine O")
+    check_close(LSE, LSE_ref, 1e-5, what="combine LSE")
+
+
+# --------------------------------------------------------------------------- a1 scores
+@pytest.mark.parametrize("name,kw", [
+    ("tiny", {}),
+    ("tiny", dict(C=127, L_q=16)),                   # Cp = 128: exactly one full tile
+    ("tiny", dict(C=130, N=5, K=2)),                 # Cp = 131: full tile + 3-row tail (16-row TMA box)
+    ("tiny", dict(C=200, H=8, H_kv=2, L_q=40, L_d=8)),   # GQA G=4, 160 scoring rows -> 2 M tiles (atomic path)
+    ("llada8k", {}),
+    ("dream16k", {}),
+])
+def test_scores(B, name, kw):
+    w, inp = _inputs(name, **kw)
+    shape = B.Shape.of(w)
+    got = B.score_chunks(shape, dev_bf16(inp["Q_dec"]), dev_bf16(inp["Kcache"]))
+    ref = oracle.scores(inp["Q_dec"], inp["Kcache"], w.L_q)
+    err = check_close(got, ref, SCORE_ABS, what="scores")
+    ids = B.select_topk(shape, got)
+    check_exact(ids, oracle.topk(ref, w.K))
+    if not kw:
+        check_exact(ids, inp["planted"], "planted chunks")
+    print(f"{name} {kw}: scores max|d| = {err:.2e}")
+
+
+# --------------------------------------------------------------------------- a3+a4+a5 attention
+def _attn_case(B, w, inp, splits, ids=None):
+    dev = to_device(inp)
+    ids = inp["planted"] if ids is None else ids
+    shape = shape_of(inp, ids.shape[-1], w.L_q)
+    O_ref, LSE_ref = oracle.attn(inp["Q_dec"], inp["Kcache"], inp["Vcache"], ids, inp["keep"], inp["K_dec"], inp["V_dec"])
+    gi_ref = oracle.gather_idx(ids, inp["keep"], w.N, w.C)
+    for S in splits:
+        gi = torch.empty(gi_ref.shape, dtype=torch.int32, device="cuda")
+        O, LSE = B.sparse_attn(shape, dev["Q_dec"], dev["Kcache"], dev["Vcache"], dev_i32(ids), dev["keep"],
+                               dev["K_dec"], dev["V_dec"], n_splits=S, gather_idx_out=gi)
+        torch.cuda.synchronize()
+        e_o, r_o = check_O(O, O_ref, what=f"O (S={S})")
+        e_l = check_close(LSE, LSE_ref, LSE_ABS, what=f"LSE (S={S})")
+        check_exact(gi, gi_ref, "gather_idx")
+        print(f"{w.name} S={S}: O max|d| {e_o:.2e} (norm {r_o:.2e}), LSE max|d| {e_l:.2e}")
+
+
+def test_attn_tiny(B):
+    w, inp = _inputs("tiny")
+    _attn_case(B, w, inp, [1, 2, 4, 0])
+
+
+@pytest.mark.parametrize("kw", [
+    dict(keep=1.0),                                   # no keep list (NULL)
+    dict(K=8, keep=1.0),                              # K = N, full mask: dense attention over the whole prefix
+    dict(keep=0.0),                                   # only the BOS of each selected chunk survives (Bk = 1)
+    dict(L_q=1, L_d=0),                               # a single query row, L_s = 1
+    dict(L_q=100, L_d=101, C=100, keep=0.37),         # ragged everything: L = 201, Bk = 38
+    dict(H=8, H_kv=2, L_q=20, L_d=30),                # GQA G=4: 200 packed rows, tiles straddle heads
+    dict(B=3, H=6, H_kv=3, d=128, C=96, L_q=8, L_d=24),
+])
+def test_attn_edges(B, kw):
+    w, inp = _inputs("tiny", **kw)
+    _attn_case(B, w, inp, [1, 3, 64])
+
+
+def test_attn_llada8k(B):
+    w, inp = _inputs("llada8k")
+    _attn_case(B, w, inp, [0, 1, 4])
+
+
+def test_attn_dream16k_split_sweep(B):
+    w, inp = _inputs("dream16k")
+    _attn_case(B, w, inp, [1, 2, 3, 5, 8, 20, 64, 0])
+
+
+def test_attn_large_logits(B):
+    """A key with logit ~ +50 above the rest (oracle pin iv) and strongly growing maxima across KV tiles:
+    exercises the reference-max update and the O rescale."""
+    w, inp = _inputs("tiny", C=300, L_q=64, L_d=64, keep=1.0)
+    u = np.zeros(w.d, np.float32); u[::2] = 1.0; u /= np.linalg.norm(u)
+    Q = W.bf16_bits_to_f32(inp["Q_dec"]) + 4.0 * u                                # logit = (1/8) * 4 * 20 * ramp
+    Kc = W.bf16_bits_to_f32(inp["Kcache"]).copy()
+    ramp = np.linspace(0.0, 6.0, w.N * w.Cp, dtype=np.float32).reshape(w.N, w.Cp, 1)
+    Kc += (20.0 * ramp * u)[None, None]
+    inp["Q_dec"], inp["Kcache"] = W.f32_to_bf16_bits(Q), W.f32_to_bf16_bits(Kc)
+    _attn_case(B, w, inp, [1, 2])
+
+
+# --------------------------------------------------------------------------- the per-step call
+def test_step_tiny(B):
+    w, inp = _inputs("tiny")
+    dev = to_device(inp)
+    shape = B.Shape.of(w)
+    ref = oracle.step(inp["Q_dec"], inp["Kcache"], inp["Vcache"], inp["keep"], inp["K_dec"], inp["V_dec"], w.K, w.L_q)
+    for S in (1, 2, 4):
+        out = B.step(shape, dev["Q_dec"], dev["Kcache"], dev["Vcache"], dev["keep"], dev["K_dec"], dev["V_dec"], n_splits=S)
+        torch.cuda.synchronize()
+        check_close(out["scores"], ref["scores"], SCORE_ABS, what="scores")
+        check_exact(out["chunk_ids"], ref["ids"])
+        check_O(out["O"], ref["O"])
+        check_close(out["LSE"], ref["LSE"], LSE_ABS)
+
+
+def test_step_sparse32k_full_size_sampled(B):
+    """BASELINE configs[3] at full size in bench.py's launch configuration (n_splits = 0); the oracle
+    checks sampled (b, head) slices one by one."""
+    w, inp = _inputs("sparse32k")
+    dev = to_device(inp)
+    shape = B.Shape.of(w)
+    gi = torch.empty((w.B, w.H_kv, w.K * w.Bk), dtype=torch.int32, device="cuda")
+    out = B.step(shape, dev["Q_dec"], dev["Kcache"], dev["Vcache"], dev["keep"], dev["K_dec"], dev["V_dec"],
+                 n_splits=0, gather_idx_out=gi)
+    torch.cuda.synchronize()
+    check_exact(out["chunk_ids"], inp["planted"], "planted chunks (all heads)")
+    r = np.random.default_rng(7)
+    sample = [(0, 0), (w.B - 1, w.H - 1)] + [(int(r.integers(w.B)), int(r.integers(w.H))) for _ in range(6)]
+    for b, h in sample:
+        sl = lambda a: a[b:b + 1, h:h + 1]
+        sc = oracle.scores(sl(inp["Q_dec"]), sl(inp["Kcache"]), w.L_q)
+        ids = oracle.topk(sc, w.K)
+        check_close(out["scores"][b:b + 1, h:h + 1], sc, SCORE_ABS, what=f"scores[{b},{h}]")
+        check_exact(out["chunk_ids"][b:b + 1, h:h + 1], ids, f"ids[{b},{h}]")
+        check_exact(gi[b:b + 1, h:h + 1], oracle.gather_idx(ids, sl(inp["keep"]), w.N, w.C), f"gather_idx[{b},{h}]")
+        O_ref, LSE_ref = oracle.attn(sl(inp["Q_dec"]), sl(inp["Kcache"]), sl(inp["Vcache"]), ids, sl(inp["keep"]),
+                                     sl(inp["K_dec"]), sl(inp["V_dec"]))
+        check_O(out["O"][b:b + 1, h:h + 1], O_ref, what=f"O[{b},{h}]")
+        check_close(out["LSE"][b:b + 1, h:h + 1], LSE_ref, LSE_ABS, what=f"LSE[{b},{h}]")
+
+
+def test_step_host_matches_step(B):
+    """pdllm_step_host (pinned host buffers, copies on the stream) returns what pdllm_step computes."""
+    w, inp = _inputs("tiny")
+    dev = to_device(inp)
+    shape = B.Shape.of(w)
+    pin = lambda bits: torch.from_numpy(bits.view(np.int16)).view(torch.bfloat16).pin_memory()
+    hQ, hK, hV = pin(inp["Q_dec"]), pin(inp["K_dec"]), pin(inp["V_dec"])
+    hO = torch.empty((w.B, w.H, w.L, w.d), dtype=torch.bfloat16).pin_memory()
+    hL = torch.empty((w.B, w.H, w.L), dtype=torch.float32).pin_memory()
+    hI = torch.empty((w.B, w.H_kv, w.K), dtype=torch.int32).pin_memory()
+    scratch = torch.empty((B.step_host_scratch_bytes(shape, 2, B.num_sms()),), dtype=torch.uint8, device="cuda")
+    B.step_host(shape, hQ, hK, hV, dev["Kcache"], dev["Vcache"], dev["keep"], 2, hO, hL, hI, scratch)
+    torch.cuda.synchronize()
+    out = B.step(shape, dev["Q_dec"], dev["Kcache"], dev["Vcache"], dev["keep"], dev["K_dec"], dev["V_dec"], n_splits=2)
+    torch.cuda.synchronize()
+    assert torch.equal(hO.view(torch.int16), out["O"].cpu().view(torch.int16))
+    assert torch.equal(hL, out["LSE"].cpu())
+    assert torch.equal(hI, out["chunk_ids"].cpu())
+
+
+def test_errors(B):
+    w, inp = _inputs("tiny", C=300, keep=1.0)        # S_kv = 650: several KV tiles, so 2 splits need scratch
+    dev = to_device(inp)
+    shape = B.Shape.of(w)
+    bad = B.Shape(w.B, w.H, 3, w.d, w.N, w.C, w.K, w.Bk, w.L_q, w.L, w.L_s)       # H % H_kv != 0
+    with pytest.raises(B.PdllmError):
+        B.select_topk(bad, torch.zeros((1, 3, w.N), device="cuda"))
+    ws = torch.empty((16,), dtype=torch.uint8, device="cuda")
+    with pytest.raises(B.PdllmError):                                             # workspace too small for 2 splits
+        B.sparse_attn(shape, dev["Q_dec"], dev["Kcache"], dev["Vcache"], dev_i32(inp["planted"]), dev["keep"],
+                      dev["K_dec"], dev["V_dec"], n_splits=2, workspace=ws)
