@@ -1,0 +1,391 @@
+#!/usr/bin/env python
+"""bench.py -- per-denoising-step sparse attention of Prefilling-dLLM on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload NAME]
+
+A "step" is one pass of the whole hot path (chunk-score reduction -> top-K -> index-driven
+gather + Split-S partial attention -> LSE combine) over one batch of seeded synthetic input, i.e. one
+`pdllm_step` call through the C ABI.  Default workload: BASELINE.json configs[3] ("32K long-context
+sparse", the configuration the metric is quoted on; it fits one GPU).
+
+Prints ONE JSON line (rank 0): `value` = device-timed us per step with inputs resident in HBM;
+`e2e` = the same through `pdllm_step_host` with pinned HOST per-step tensors (H2D + D2H inside the timed
+region); `roofline` for the dominant kernel (per-stage CUDA events recorded inside the timed region by
+`pdllm_step_profiled`); `cpu_baseline` = the fp64 oracle timed on this box's host cores on a bounded
+sample.  `--impl reference` times the oracle alone (there is no reference code: /root/reference holds a
+paper only).
+
+Multi-GPU: replicas only -- the path is fixed to one GPU by BASELINE.json; under
+torchrun every rank runs an independent replica of the step, time = max over ranks.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import sys
+import threading
+import time
+from pathlib import Path
+
+import numpy as np
+
+ROOT = Path(__file__).resolve().parent
+sys.path.insert(0, str(ROOT))
+
+from paper_2606_10537_b200 import workloads as W  # noqa: E402
+
+METRIC = "us_per_denoising_step_attention"
+UNIT = "us"
+FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture
+# (profiles/), keyed by (workload, kernel); None until a capture exists for that pair.
+NCU_TRAFFIC_BYTES = {}
+
+
+def load_peaks():
+    p = ROOT / "MEASURED_PEAKS.json"
+    if p.exists():
+        try:
+            d = json.loads(p.read_text())
+            return {k: float(d[k]) for k in FALLBACK_PEAKS if k in d} | {"source": "measured"}
+        except Exception:
+            pass
+    return dict(FALLBACK_PEAKS, source="fallback")
+
+
+# --------------------------------------------------------------------------- clocks during the timed region
+class ClockSampler:
+    """Samples SM clock and throttle reasons with NVML every few ms while the timed region runs."""
+    BAD = {"hw_slowdown": 0x8, "sw_thermal_slowdown": 0x20, "hw_thermal_slowdown": 0x40}
+    NOTE = {"sw_power_cap": 0x4, "hw_power_brake": 0x80}
+
+    def __init__(self, index: int, period_s: float = 0.004):
+        self.index, self.period = index, period_s
+        self.samples, self.reasons = [], 0
+        self._stop = threading.Event()
+        self._thr = None
+        self.max_mhz = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def _reasons(self):
+        for fn in ("nvmlDeviceGetCurrentClocksEventReasons", "nvmlDeviceGetCurrentClocksThrottleReasons"):
+            f = getattr(self.nv, fn, None)
+            if f is not None:
+                try:
+                    return int(f(self.h))
+                except Exception:
+                    continue
+        return 0
+
+    def _run(self):
+        while not self._stop.is_set():
+            try:
+                self.samples.append(self.nv.nvmlDeviceGetClockInfo(self.h, self.nv.NVML_CLOCK_SM))
+                self.reasons |= self._reasons()
+            except Exception:
+                pass
+            self._stop.wait(self.period)
+
+    def __enter__(self):
+        if self.nv is not None:
+            self._thr = threading.Thread(target=self._run, daemon=True)
+            self._thr.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        if self._thr is not None:
+            self._thr.join()
+
+    def summary(self):
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": ["unavailable"]}
+        names = [n for n, bit in {**self.BAD, **self.NOTE}.items() if self.reasons & bit]
+        return {"sm_mhz": statistics.median(self.samples), "sm_max_mhz": self.max_mhz, "reasons": names,
+                "samples": len(self.samples)}
+
+
+# --------------------------------------------------------------------------- the oracle leg (CPU baseline / reference arm)
+def oracle_sample(w: W.Workload, inp: dict, threads: int):
+    """A bounded sample of the workload for the oracle: the first n KV groups of batch element 0 (with their
+    G query heads each), one group per host thread.  Returns (slices, scale-up factor to the whole step)."""
+    n = max(1, min(w.H_kv, threads // max(1, min(w.G, threads))))
+    sl = dict(Q_dec=np.ascontiguousarray(inp["Q_dec"][:1, : n * w.G]), Kcache=np.ascontiguousarray(inp["Kcache"][:1, :n]),
+              Vcache=np.ascontiguousarray(inp["Vcache"][:1, :n]), K_dec=np.ascontiguousarray(inp["K_dec"][:1, :n]),
+              V_dec=np.ascontiguousarray(inp["V_dec"][:1, :n]),
+              keep=None if inp["keep"] is None else np.ascontiguousarray(inp["keep"][:1, :n]))
+    return sl, n, (w.B * w.H_kv) / n
+
+
+def time_oracle_once(w, sl):
+    from oracle import oracle
+    t0 = time.perf_counter()
+    oracle.step(sl["Q_dec"], sl["Kcache"], sl["Vcache"], sl["keep"], sl["K_dec"], sl["V_dec"], w.K, w.L_q)
+    return time.perf_counter() - t0
+
+
+def time_oracle_pieces(w, sl, n_chunks, ids):
+    """The oracle's step on the sample with the scoring restricted to the first n_chunks chunks (each chunk's
+    score is independent of the others): returns (seconds scoring n_chunks chunks, seconds for the rest =
+    top-K + gather indices + concatenation + attention with the selected ids)."""
+    from oracle import oracle
+    t0 = time.perf_counter()
+    sc = oracle.scores(sl["Q_dec"], np.ascontiguousarray(sl["Kcache"][:, :, :n_chunks]), w.L_q)
+    t1 = time.perf_counter()
+    oracle.topk(sc, min(w.K, n_chunks))
+    oracle.gather_idx(ids, sl["keep"], w.N, w.C)
+    oracle.attn(sl["Q_dec"], sl["Kcache"], sl["Vcache"], ids, sl["keep"], sl["K_dec"], sl["V_dec"])
+    t2 = time.perf_counter()
+    return t1 - t0, t2 - t1
+
+
+def run_reference(args, w):
+    """--impl reference: the oracle, as it stands, on the host cores (rank 0 only).  Each step times a bounded
+    sample (some (batch, KV-head) groups; the scoring over some of the N chunks) and scales it to the whole
+    step; the sample is sized so that steps + warmup end within a few minutes."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    from oracle import oracle
+    cores = oracle.num_threads()
+    inp = W.make_inputs(W.small_variant(w, B=1))      # the sample only touches batch element 0
+    sl, n, factor = oracle_sample(w, inp, cores)
+    ids = np.ascontiguousarray(inp["planted"][:1, :n])
+    t_s1, t_rest = time_oracle_pieces(w, sl, 1, ids)  # probe: one chunk
+    budget = max(0.05, 150.0 / max(1, args.steps + args.warmup))
+    n_chunks = int(max(1, min(w.N, (budget - t_rest) / max(t_s1, 1e-6))))
+    for _ in range(args.warmup):
+        time_oracle_pieces(w, sl, n_chunks, ids)
+    tot = 0.0
+    for _ in range(args.steps):
+        ts, tr = time_oracle_pieces(w, sl, n_chunks, ids)
+        tot += ts * (w.N / n_chunks) + tr
+    us = 1e6 * factor * tot / max(1, args.steps)
+    sample = (f"per step: {n} of {w.B * w.H_kv} (batch, KV-head) groups (b=0, groups 0..{n - 1}, {w.G} query head(s) each); "
+              f"scoring over {n_chunks} of {w.N} chunks scaled x{w.N / n_chunks:g}, attention in full; "
+              f"whole sample scaled x{factor:g} to the step")
+    line = {"impl": "reference", "metric": METRIC, "value": us, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": us / 1e3, "higher_is_better": False, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": workload_config(w, None),
+            "cpu_baseline": {"value": us, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": us, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def workload_config(w, n_splits):
+    return {"workload": f"BASELINE.json configs[{list(W.CONFIGS).index(w.name)}] '{w.name}'", "B": w.B, "H": w.H,
+            "H_kv": w.H_kv, "d": w.d, "N": w.N, "C": w.C, "K": w.K, "keep": w.keep, "Bk": w.Bk, "L_q": w.L_q,
+            "L_d": w.L_d, "prefix_tokens": w.N * w.C, "n_splits": n_splits,
+            "call": "pdllm_step (score_chunks -> select_topk -> sparse_attn -> lse_combine)",
+            "l2": "inputs larger than L2: the step streams the whole K cache "
+                  f"({w.score_bytes() / 1e6:.0f} MB) every iteration; no explicit flush"}
+
+
+# --------------------------------------------------------------------------- our arm
+def run_ours(args, w):
+    import torch
+    import torch.distributed as dist
+    from paper_2606_10537_b200 import binding as B
+
+    rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the pdllm hot path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    B.lib()
+    sms = B.num_sms()
+    shape = B.Shape.of(w)
+    inp = W.make_inputs(w)
+    bf = lambda bits: torch.from_numpy(np.ascontiguousarray(bits).view(np.int16)).cuda().view(torch.bfloat16)
+    dQ, dKc, dVc, dKd, dVd = (bf(inp[k]) for k in ("Q_dec", "Kcache", "Vcache", "K_dec", "V_dec"))
+    dkeep = None if inp["keep"] is None else torch.from_numpy(inp["keep"]).cuda()
+    S = args.n_splits if args.n_splits > 0 else B.auto_splits(shape, sms)
+    ws = B.alloc_workspace(shape, args.n_splits)
+    out = dict(scores=torch.empty((w.B, w.H_kv, w.N), dtype=torch.float32, device="cuda"),
+               chunk_ids=torch.empty((w.B, w.H_kv, w.K), dtype=torch.int32, device="cuda"),
+               O=torch.empty((w.B, w.H, w.L, w.d), dtype=torch.bfloat16, device="cuda"),
+               LSE=torch.empty((w.B, w.H, w.L), dtype=torch.float32, device="cuda"))
+
+    def step(events=None):
+        B.step(shape, dQ, dKc, dVc, dkeep, dKd, dVd, n_splits=args.n_splits, workspace=ws, events=events, **out)
+
+    K, Wm = args.steps, args.warmup
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(5)] for _ in range(K)]
+    for row in evs:                       # torch creates the cudaEvent_t on first record
+        for e in row:
+            e.record()
+    for _ in range(Wm):
+        step()
+    torch.cuda.synchronize()
+    ok = bool((out["chunk_ids"].cpu().numpy() == inp["planted"]).all())     # sanity: the planted chunks are found
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    t_begin, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    with ClockSampler(local) as clk:
+        t_begin.record()
+        for k in range(K):
+            step(evs[k])
+        t_end.record()
+        barrier()
+    total_ms = t_begin.elapsed_time(t_end)
+    if world > 1:
+        t = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    # replicas: world independent steps ran per iteration
+    us_per_step = 1e3 * total_ms / (K * world)
+
+    def stage(i, j):
+        return 1e3 * sum(evs[k][i].elapsed_time(evs[k][j]) for k in range(K)) / K
+    t_score, t_topk, t_attn, t_comb = stage(0, 1), stage(1, 2), stage(2, 3), stage(3, 4)
+
+    # the same loop without per-stage events (what a user runs): reported beside, not as `value`
+    barrier()
+    t_begin.record()
+    for _ in range(K):
+        step()
+    t_end.record()
+    barrier()
+    us_plain = 1e3 * t_begin.elapsed_time(t_end) / K
+
+    # the paper's static-selection mode: per step only pdllm_sparse_attn
+    ids = out["chunk_ids"].clone()
+    barrier()
+    t_begin.record()
+    for _ in range(K):
+        B.sparse_attn(shape, dQ, dKc, dVc, ids, dkeep, dKd, dVd, n_splits=args.n_splits, O=out["O"], LSE=out["LSE"],
+                      workspace=ws)
+    t_end.record()
+    barrier()
+    us_attn_only = 1e3 * t_begin.elapsed_time(t_end) / K
+
+    # ---- e2e: HOST per-step tensors through pdllm_step_host, copies inside the timed region
+    pin = lambda bits: torch.from_numpy(np.ascontiguousarray(bits).view(np.int16)).view(torch.bfloat16).pin_memory()
+    hQ, hK, hV = pin(inp["Q_dec"]), pin(inp["K_dec"]), pin(inp["V_dec"])
+    hO = torch.empty((w.B, w.H, w.L, w.d), dtype=torch.bfloat16).pin_memory()
+    hL = torch.empty((w.B, w.H, w.L), dtype=torch.float32).pin_memory()
+    hI = torch.empty((w.B, w.H_kv, w.K), dtype=torch.int32).pin_memory()
+    scratch = torch.empty((B.step_host_scratch_bytes(shape, args.n_splits, sms),), dtype=torch.uint8, device="cuda")
+    stream = torch.cuda.current_stream()
+
+    def host_step():
+        B.step_host(shape, hQ, hK, hV, dKc, dVc, dkeep, args.n_splits, hO, hL, hI, scratch)
+        stream.synchronize()              # the caller reads O / LSE / ids after every step
+
+    for _ in range(Wm):
+        host_step()
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(K):
+        host_step()
+    barrier()
+    e2e_s = time.perf_counter() - t0
+    if world > 1:
+        t = torch.tensor([e2e_s], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    e2e_us = 1e6 * e2e_s / (K * world)
+    h2d = hQ.numel() * 2 + hK.numel() * 2 + hV.numel() * 2
+    d2h = hO.numel() * 2 + hL.numel() * 4 + hI.numel() * 4
+    e2e_ok = bool((hI.numpy() == inp["planted"]).all())
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel + the attention kernel (algorithmic work: DESIGN.md "Measurement")
+    peaks = load_peaks()
+    score_gbs = w.score_bytes() / (t_score * 1e-6) / 1e9
+    score_tf = w.score_flops() / (t_score * 1e-6) / 1e12
+    attn_t = t_attn + t_comb
+    attn_tf = w.attn_flops() / (attn_t * 1e-6) / 1e12
+    attn_gbs = w.attn_bytes() / (attn_t * 1e-6) / 1e9
+    roof_score = {"kernel": "score_kernel (a1)", "bound": "hbm", "achieved": score_gbs, "peak": peaks["hbm_gbs"],
+                  "unit": "GB/s", "frac": score_gbs / peaks["hbm_gbs"], "peak_source": peaks["source"],
+                  "traffic": NCU_TRAFFIC_BYTES.get((w.name, "score_kernel")), "us": t_score,
+                  "algorithmic_bytes": w.score_bytes()}
+    t_tensor = w.attn_flops() / (peaks["bf16_tflops_sustained"] * 1e12)
+    t_hbm = w.attn_bytes() / (peaks["hbm_gbs"] * 1e9)
+    attn_bound = "tensor" if t_tensor >= t_hbm else "hbm"
+    roof_attn = {"kernel": "attn_kernel (a3+a4)" + (" + combine_kernel (a5)" if S > 1 else ""), "bound": attn_bound,
+                 "achieved": attn_tf if attn_bound == "tensor" else attn_gbs,
+                 "peak": peaks["bf16_tflops_sustained"] if attn_bound == "tensor" else peaks["hbm_gbs"],
+                 "unit": "TFLOP/s" if attn_bound == "tensor" else "GB/s",
+                 "frac": max(t_tensor, t_hbm) / (attn_t * 1e-6), "peak_source": peaks["source"] + " (sustained)",
+                 "traffic": NCU_TRAFFIC_BYTES.get((w.name, "attn_kernel")), "us": attn_t,
+                 "tflops": attn_tf, "gbs": attn_gbs, "roofline_us": 1e6 * max(t_tensor, t_hbm)}
+    dominant = roof_score if t_score >= attn_t else roof_attn
+    step_flops = w.score_flops() + w.attn_flops()
+    step_bytes = w.score_bytes() + w.attn_bytes() + w.topk_bytes()
+    roof_step_us = 1e6 * max(step_flops / (peaks["bf16_tflops_sustained"] * 1e12), step_bytes / (peaks["hbm_gbs"] * 1e9))
+
+    # ---- the oracle on this box's host cores (bounded sample)
+    from oracle import oracle
+    cores = oracle.num_threads()
+    sl, n, factor = oracle_sample(w, inp, cores)
+    reps = 3
+    t_or = min(time_oracle_once(w, sl) for _ in range(reps))
+    cpu = {"value": 1e6 * t_or * factor, "unit": UNIT, "cores": cores, "kind": "oracle",
+           "sample": f"{n} of {w.B * w.H_kv} (batch, KV-head) groups (b=0, groups 0..{n - 1}), best of {reps}, "
+                     f"time scaled x{factor:g} to the whole step"}
+
+    clocks = clk.summary()
+    line = {"metric": METRIC, "value": us_per_step, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
+            "ms_per_step": us_per_step / 1e3, "higher_is_better": False,
+            "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+            "config": workload_config(w, S),
+            "tflops": step_flops / (us_per_step * world * 1e-6) / 1e12,
+            "gbs": step_bytes / (us_per_step * world * 1e-6) / 1e9,
+            "step_roofline": {"us": roof_step_us, "frac": roof_step_us / (us_per_step * world),
+                              "peak_source": peaks["source"]},
+            "stages_us": {"score_chunks": t_score, "select_topk": t_topk, "sparse_attn_partial": t_attn,
+                          "lse_combine": t_comb, "step_without_stage_events": us_plain,
+                          "sparse_attn_only_static_selection": us_attn_only},
+            "roofline": dominant, "roofline_attn": roof_attn, "roofline_score": roof_score,
+            "e2e": {"value": e2e_us, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                    "call": "pdllm_step_host (pinned host Q_dec/K_dec/V_dec in; O, LSE, chunk ids out; KV cache resident)",
+                    "result_ok": e2e_ok},
+            "gpu_launches": K * (3 + (1 if S > 1 else 0)),
+            "cpu_baseline": cpu, "clocks": clocks, "planted_chunks_recovered": ok}
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
+    ap.add_argument("--workload", choices=list(W.CONFIGS), default="sparse32k")
+    ap.add_argument("--n-splits", type=int, default=0, help="0 = pdllm_auto_splits")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    w = W.CONFIGS[args.workload]
+    if args.impl == "reference":
+        run_reference(args, w)
+    else:
+        run_ours(args, w)
+
+
+if __name__ == "__main__":
+    main()

@@ -160,6 +160,26 @@ int pdllm_step(const pdllm_shape *shape, const void *Q_dec, const void *Kcache, 
                int32_t *gather_idx_out, void *workspace, size_t workspace_bytes,
                pdllm_stream_t stream);
 
+/* ---- pdllm_step with per-stage timestamps (measurement aid, S8(d)) ---------------
+ * Same enqueue sequence as pdllm_step; additionally records the given CUDA events
+ * (cudaEvent_t handles created by the caller with timing enabled, passed as opaque
+ * pointers; a NULL member is skipped) on `stream` at the stage boundaries, so that
+ * a harness can attribute the step's device time to a1 / a2 / a3-a5 inside the same
+ * timed region.  ev == NULL is exactly pdllm_step. */
+typedef struct {
+    void *begin;         /* before a1 */
+    void *after_score;   /* after a1 (chunk-score reduction) */
+    void *after_topk;    /* after a2 (top-K) */
+    void *after_attn;    /* after a3+a4 (Split-S partial attention), before a5 */
+    void *end;           /* after a5 (LSE combine; == after_attn time when one split) */
+} pdllm_stage_events;
+
+int pdllm_step_profiled(const pdllm_shape *shape, const void *Q_dec, const void *Kcache, const void *Vcache,
+                        const int32_t *token_keep_idx, const void *K_dec, const void *V_dec, int32_t n_splits,
+                        float *scores_out, int32_t *chunk_ids_out, void *O, float *LSE,
+                        int32_t *gather_idx_out, void *workspace, size_t workspace_bytes,
+                        const pdllm_stage_events *ev, pdllm_stream_t stream);
+
 /* ---- the per-step call with HOST per-step tensors ------------------------------
  * The prefix cache and keep lists are state that the prefill left on the device
  * ("static cache that is reused across all T denoising steps"); what

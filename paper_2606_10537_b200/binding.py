@@ -20,13 +20,17 @@ _lib = None
 EXPORTS = [
     "pdllm_version", "pdllm_strerror", "pdllm_auto_splits", "pdllm_workspace_bytes",
     "pdllm_step_host_scratch_bytes", "pdllm_score_chunks", "pdllm_select_topk", "pdllm_gather_idx",
-    "pdllm_sparse_attn", "pdllm_lse_combine", "pdllm_step", "pdllm_step_host",
+    "pdllm_sparse_attn", "pdllm_lse_combine", "pdllm_step", "pdllm_step_profiled", "pdllm_step_host",
 ]
 
 
 class PdllmShape(ctypes.Structure):
     _fields_ = [(n, ctypes.c_int32) for n in ("B", "H", "H_kv", "d", "N", "C", "K", "Bk", "L_q", "L", "L_s")] + [
         ("scale", ctypes.c_float)]
+
+
+class PdllmStageEvents(ctypes.Structure):
+    _fields_ = [(n, ctypes.c_void_p) for n in ("begin", "after_score", "after_topk", "after_attn", "end")]
 
 
 @dataclass(frozen=True)
@@ -87,9 +91,11 @@ def lib() -> ctypes.CDLL:
     L.pdllm_sparse_attn.argtypes = [shp, vp, vp, vp, vp, vp, vp, vp, i32, vp, vp, vp, vp, sz, vp]
     L.pdllm_lse_combine.argtypes = [vp, vp, i32, i64, i32, vp, vp, vp]
     L.pdllm_step.argtypes = [shp, vp, vp, vp, vp, vp, vp, i32, vp, vp, vp, vp, vp, vp, sz, vp]
+    L.pdllm_step_profiled.argtypes = [shp, vp, vp, vp, vp, vp, vp, i32, vp, vp, vp, vp, vp, vp, sz,
+                                      ctypes.POINTER(PdllmStageEvents), vp]
     L.pdllm_step_host.argtypes = [shp, vp, vp, vp, vp, vp, vp, i32, vp, vp, vp, vp, sz, vp]
     for n in ("pdllm_score_chunks", "pdllm_select_topk", "pdllm_gather_idx", "pdllm_sparse_attn", "pdllm_lse_combine",
-              "pdllm_step", "pdllm_step_host"):
+              "pdllm_step", "pdllm_step_profiled", "pdllm_step_host"):
         getattr(L, n).restype = ctypes.c_int
     _lib = L
     return L
@@ -200,8 +206,12 @@ def lse_combine(O_part, lse_part, O=None, LSE=None, stream=None):
 
 
 def step(shape: Shape, Q_dec, Kcache, Vcache, token_keep_idx, K_dec, V_dec, n_splits=0, scores=None, chunk_ids=None,
-         O=None, LSE=None, gather_idx_out=None, workspace=None, stream=None):
-    """One denoising step's attention: score_chunks -> select_topk -> sparse_attn (-> combine)."""
+         O=None, LSE=None, gather_idx_out=None, workspace=None, stream=None, events=None):
+    """One denoising step's attention: score_chunks -> select_topk -> sparse_attn (-> combine).
+
+    events: optional 5 torch.cuda.Event(enable_timing=True), each recorded at least once before (torch creates the
+    cudaEvent_t lazily); pdllm_step_profiled records them at the stage boundaries (begin, after_score, after_topk,
+    after_attn, end) on the stream."""
     torch = _torch()
     dev = Q_dec.device
     if scores is None:
@@ -214,9 +224,14 @@ def step(shape: Shape, Q_dec, Kcache, Vcache, token_keep_idx, K_dec, V_dec, n_sp
         LSE = torch.empty((shape.B, shape.H, shape.L), dtype=torch.float32, device=dev)
     if workspace is None:
         workspace = alloc_workspace(shape, n_splits, dev)
-    _check(lib().pdllm_step(ctypes.byref(shape.c()), _ptr(Q_dec), _ptr(Kcache), _ptr(Vcache), _ptr(token_keep_idx),
-                            _ptr(K_dec), _ptr(V_dec), n_splits, _ptr(scores), _ptr(chunk_ids), _ptr(O), _ptr(LSE),
-                            _ptr(gather_idx_out), _ptr(workspace), workspace.numel(), _stream(stream)))
+    args = (ctypes.byref(shape.c()), _ptr(Q_dec), _ptr(Kcache), _ptr(Vcache), _ptr(token_keep_idx),
+            _ptr(K_dec), _ptr(V_dec), n_splits, _ptr(scores), _ptr(chunk_ids), _ptr(O), _ptr(LSE),
+            _ptr(gather_idx_out), _ptr(workspace), workspace.numel())
+    if events is None:
+        _check(lib().pdllm_step(*args, _stream(stream)))
+    else:
+        ev = PdllmStageEvents(*[ctypes.c_void_p(e.cuda_event) for e in events])
+        _check(lib().pdllm_step_profiled(*args, ctypes.byref(ev), _stream(stream)))
     return dict(scores=scores, chunk_ids=chunk_ids, O=O, LSE=LSE)
 
 

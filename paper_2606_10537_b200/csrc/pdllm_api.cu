@@ -171,21 +171,17 @@ int pdllm_lse_combine(const float *O_part, const float *lse_part, int32_t S, int
     return cuda_rc(launch_combine(O_part, lse_part, S, rows, d, O, LSE, static_cast<cudaStream_t>(stream)));
 }
 
-int pdllm_sparse_attn(const pdllm_shape *shape, const void *Q_dec, const void *Kcache, const void *Vcache,
-                      const int32_t *chunk_ids, const int32_t *token_keep_idx, const void *K_dec, const void *V_dec,
-                      int32_t n_splits, void *O, float *LSE, int32_t *gather_idx_out, void *workspace,
-                      size_t workspace_bytes, pdllm_stream_t stream) {
-    if (!shape || !Q_dec || !Kcache || !Vcache || !chunk_ids || !K_dec || !V_dec || !O || !LSE) return PDLLM_ERR_NULL;
-    if (n_splits < 0) return PDLLM_ERR_SHAPE;
-    Dims d;
-    if (int rc = resolve(shape, token_keep_idx != nullptr, &d)) return rc;
-    if (!aligned16(Q_dec) || !aligned16(Kcache) || !aligned16(Vcache) || !aligned16(K_dec) || !aligned16(V_dec) ||
-        !aligned16(O) || !aligned16(workspace))
-        return PDLLM_ERR_ALIGN;
-    cudaStream_t st = static_cast<cudaStream_t>(stream);
-    const int S = effective_splits(d, n_splits, device_num_sms());
-    const size_t need = workspace_for(d, S);
-    if (need > 0 && (!workspace || workspace_bytes < need)) return PDLLM_ERR_WORKSPACE;
+namespace {
+
+int record(void *ev, cudaStream_t st) {
+    if (!ev) return PDLLM_OK;
+    return cuda_rc(cudaEventRecord(static_cast<cudaEvent_t>(ev), st));
+}
+
+// a3 + a4 + a5 on validated arguments; ev_mid / ev_end (may be NULL) are recorded after a4 / a5.
+int attn_impl(const Dims &d, const void *Q_dec, const void *Kcache, const void *Vcache, const int32_t *chunk_ids,
+              const int32_t *token_keep_idx, const void *K_dec, const void *V_dec, int S, void *O, float *LSE,
+              int32_t *gather_idx_out, void *workspace, void *ev_mid, void *ev_end, cudaStream_t st) {
     if (gather_idx_out)
         if (int rc = cuda_rc(launch_gather_idx(d, chunk_ids, token_keep_idx, gather_idx_out, st))) return rc;
     const size_t rows = (size_t)d.B * d.H * d.L;
@@ -197,28 +193,72 @@ int pdllm_sparse_attn(const pdllm_shape *shape, const void *Q_dec, const void *K
     if (int rc = cuda_rc(launch_attn(d, Q_dec, Kcache, Vcache, chunk_ids, token_keep_idx, K_dec, V_dec, S, O, LSE, O_part,
                                      lse_part, st)))
         return rc;
-    if (S > 1) return cuda_rc(launch_combine(O_part, lse_part, S, (int64_t)rows, d.d, O, LSE, st));
+    if (int rc = record(ev_mid, st)) return rc;
+    if (S > 1)
+        if (int rc = cuda_rc(launch_combine(O_part, lse_part, S, (int64_t)rows, d.d, O, LSE, st))) return rc;
+    return record(ev_end, st);
+}
+
+int attn_validate(const pdllm_shape *shape, const void *Q_dec, const void *Kcache, const void *Vcache,
+                  const int32_t *chunk_ids, const int32_t *token_keep_idx, const void *K_dec, const void *V_dec,
+                  int32_t n_splits, void *O, float *LSE, void *workspace, size_t workspace_bytes, Dims *d, int *S) {
+    if (!shape || !Q_dec || !Kcache || !Vcache || !chunk_ids || !K_dec || !V_dec || !O || !LSE) return PDLLM_ERR_NULL;
+    if (n_splits < 0) return PDLLM_ERR_SHAPE;
+    if (int rc = resolve(shape, token_keep_idx != nullptr, d)) return rc;
+    if (!aligned16(Q_dec) || !aligned16(Kcache) || !aligned16(Vcache) || !aligned16(K_dec) || !aligned16(V_dec) ||
+        !aligned16(O) || !aligned16(workspace))
+        return PDLLM_ERR_ALIGN;
+    *S = effective_splits(*d, n_splits, device_num_sms());
+    const size_t need = workspace_for(*d, *S);
+    if (need > 0 && (!workspace || workspace_bytes < need)) return PDLLM_ERR_WORKSPACE;
     return PDLLM_OK;
+}
+
+}  // namespace
+
+int pdllm_sparse_attn(const pdllm_shape *shape, const void *Q_dec, const void *Kcache, const void *Vcache,
+                      const int32_t *chunk_ids, const int32_t *token_keep_idx, const void *K_dec, const void *V_dec,
+                      int32_t n_splits, void *O, float *LSE, int32_t *gather_idx_out, void *workspace,
+                      size_t workspace_bytes, pdllm_stream_t stream) {
+    Dims d;
+    int S = 1;
+    if (int rc = attn_validate(shape, Q_dec, Kcache, Vcache, chunk_ids, token_keep_idx, K_dec, V_dec, n_splits, O, LSE,
+                               workspace, workspace_bytes, &d, &S))
+        return rc;
+    return attn_impl(d, Q_dec, Kcache, Vcache, chunk_ids, token_keep_idx, K_dec, V_dec, S, O, LSE, gather_idx_out,
+                     workspace, nullptr, nullptr, static_cast<cudaStream_t>(stream));
+}
+
+int pdllm_step_profiled(const pdllm_shape *shape, const void *Q_dec, const void *Kcache, const void *Vcache,
+                        const int32_t *token_keep_idx, const void *K_dec, const void *V_dec, int32_t n_splits,
+                        float *scores_out, int32_t *chunk_ids_out, void *O, float *LSE, int32_t *gather_idx_out,
+                        void *workspace, size_t workspace_bytes, const pdllm_stage_events *ev, pdllm_stream_t stream) {
+    if (!shape || !scores_out || !chunk_ids_out) return PDLLM_ERR_NULL;
+    if (shape->L_q > shape->L) return PDLLM_ERR_SHAPE;
+    // validate the attention arguments before anything is enqueued
+    Dims d;
+    int S = 1;
+    if (int rc = attn_validate(shape, Q_dec, Kcache, Vcache, chunk_ids_out, token_keep_idx, K_dec, V_dec, n_splits, O,
+                               LSE, workspace, workspace_bytes, &d, &S))
+        return rc;
+    if (!aligned16(scores_out)) return PDLLM_ERR_ALIGN;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (int rc = record(ev ? ev->begin : nullptr, st)) return rc;
+    if (int rc = cuda_rc(launch_score(d, Q_dec, (int64_t)d.H * d.L * d.d, (int64_t)d.L * d.d, Kcache, scores_out, st)))
+        return rc;
+    if (int rc = record(ev ? ev->after_score : nullptr, st)) return rc;
+    if (int rc = cuda_rc(launch_topk(d, scores_out, chunk_ids_out, st))) return rc;
+    if (int rc = record(ev ? ev->after_topk : nullptr, st)) return rc;
+    return attn_impl(d, Q_dec, Kcache, Vcache, chunk_ids_out, token_keep_idx, K_dec, V_dec, S, O, LSE, gather_idx_out,
+                     workspace, ev ? ev->after_attn : nullptr, ev ? ev->end : nullptr, st);
 }
 
 int pdllm_step(const pdllm_shape *shape, const void *Q_dec, const void *Kcache, const void *Vcache,
                const int32_t *token_keep_idx, const void *K_dec, const void *V_dec, int32_t n_splits, float *scores_out,
                int32_t *chunk_ids_out, void *O, float *LSE, int32_t *gather_idx_out, void *workspace,
                size_t workspace_bytes, pdllm_stream_t stream) {
-    if (!shape || !scores_out || !chunk_ids_out) return PDLLM_ERR_NULL;
-    if (shape->L_q > shape->L) return PDLLM_ERR_SHAPE;
-    // validate the attention arguments before anything is enqueued
-    if (!Q_dec || !Kcache || !Vcache || !K_dec || !V_dec || !O || !LSE) return PDLLM_ERR_NULL;
-    Dims d;
-    if (int rc = resolve(shape, token_keep_idx != nullptr, &d)) return rc;
-    if (n_splits < 0) return PDLLM_ERR_SHAPE;
-    const size_t need = workspace_for(d, effective_splits(d, n_splits, device_num_sms()));
-    if (need > 0 && (!workspace || workspace_bytes < need)) return PDLLM_ERR_WORKSPACE;
-    if (int rc = pdllm_score_chunks(shape, Q_dec, (int64_t)d.H * d.L * d.d, (int64_t)d.L * d.d, Kcache, scores_out, stream))
-        return rc;
-    if (int rc = pdllm_select_topk(shape, scores_out, chunk_ids_out, stream)) return rc;
-    return pdllm_sparse_attn(shape, Q_dec, Kcache, Vcache, chunk_ids_out, token_keep_idx, K_dec, V_dec, n_splits, O, LSE,
-                             gather_idx_out, workspace, workspace_bytes, stream);
+    return pdllm_step_profiled(shape, Q_dec, Kcache, Vcache, token_keep_idx, K_dec, V_dec, n_splits, scores_out,
+                               chunk_ids_out, O, LSE, gather_idx_out, workspace, workspace_bytes, nullptr, stream);
 }
 
 int pdllm_step_host(const pdllm_shape *shape, const void *h_Q_dec, const void *h_K_dec, const void *h_V_dec,
