@@ -41,7 +41,11 @@ UNIT = "us"
 FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture
 # (profiles/), keyed by (workload, kernel); None until a capture exists for that pair.
-NCU_TRAFFIC_BYTES = {}
+NCU_TRAFFIC_BYTES = {
+    # profiles/r1_ncu_full_v0.md (kernels v0)
+    ("sparse32k", "score_kernel"): 1086.234e6 + 3.425792e6,
+    ("sparse32k", "attn_kernel"): 106.138e6 + 3.784704e6,
+}
 
 
 def load_peaks():
@@ -191,6 +195,23 @@ def workload_config(w, n_splits):
                   f"({w.score_bytes() / 1e6:.0f} MB) every iteration; no explicit flush"}
 
 
+# --------------------------------------------------------------------------- multi-rank plumbing (replicas only)
+def max_over_ranks(value: float, world: int, device="cuda") -> float:
+    """MAX all-reduce of a per-rank time; identity for one rank."""
+    if world <= 1:
+        return float(value)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([value], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def replica_us_per_step(total_ms: float, steps: int, world: int) -> float:
+    """`world` independent replicas each ran `steps` steps in total_ms (max over ranks): whole-job us per step."""
+    return 1e3 * total_ms / (steps * world)
+
+
 # --------------------------------------------------------------------------- our arm
 def run_ours(args, w):
     import torch
@@ -244,13 +265,9 @@ def run_ours(args, w):
             step(evs[k])
         t_end.record()
         barrier()
-    total_ms = t_begin.elapsed_time(t_end)
-    if world > 1:
-        t = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = max_over_ranks(t_begin.elapsed_time(t_end), world)
     # replicas: world independent steps ran per iteration
-    us_per_step = 1e3 * total_ms / (K * world)
+    us_per_step = replica_us_per_step(total_ms, K, world)
 
     def stage(i, j):
         return 1e3 * sum(evs[k][i].elapsed_time(evs[k][j]) for k in range(K)) / K
@@ -296,12 +313,8 @@ def run_ours(args, w):
     for _ in range(K):
         host_step()
     barrier()
-    e2e_s = time.perf_counter() - t0
-    if world > 1:
-        t = torch.tensor([e2e_s], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
-    e2e_us = 1e6 * e2e_s / (K * world)
+    e2e_s = max_over_ranks(time.perf_counter() - t0, world)
+    e2e_us = replica_us_per_step(1e3 * e2e_s, K, world)
     h2d = hQ.numel() * 2 + hK.numel() * 2 + hV.numel() * 2
     d2h = hO.numel() * 2 + hL.numel() * 4 + hI.numel() * 4
     e2e_ok = bool((hI.numpy() == inp["planted"]).all())
