@@ -1,80 +1,171 @@
-// attn.cu -- a3 + a4: index-driven gather of the selected BOS+chunk KV rows and the Split-S partial
-// attention kernel (R7-R11), tcgen05 / TMEM, sm_100a.
+// attn.cu -- a3 + a4 (+ the in-CTA half of a5): index-driven gather of the selected BOS+chunk KV rows and the
+// Split-S partial attention kernel (R7-R11), tcgen05 / TMEM, sm_100a.
 //
-// One CTA = one 128-row tile of the G*L query rows that share a KV head (GQA groups are packed into
-// the MMA M dimension, so K/V are read once per group) x one split of the virtual KV sequence
-//     [ K*Bk gathered cache rows  ||  L_s decode-block rows ].
-// Per 128-row KV tile:  producers (4 warps) gather K and V rows with 16-byte cp.async into
-// 128B-swizzled shared-memory panels;  one thread issues  S = Q K^T  (tcgen05.mma, SS) into TMEM;
-// the 128 softmax threads (thread = row) read S with tcgen05.ld, keep the running reference max / sum,
-// write P = exp2(.) as packed bf16 back into TMEM (aliasing S);  the MMA thread issues  O += P V
-// (tcgen05.mma, A from TMEM, V as MN-major B).  Two CTAs are resident per SM (<=113 KB smem,
-// 256 TMEM columns each) so one CTA's softmax overlaps the other's MMAs.
+// One persistent CTA per SM walks a list of work items.  An item belongs to one KV group (b, g) -- the G*L packed
+// query rows that share K/V (GQA groups sit in the MMA M dimension, so K/V are read once per group) -- and one split
+// of the virtual KV sequence [ K*Bk gathered cache rows || L_s decode-block rows ], cut at 128-row tile boundaries.
+// Every item runs TWO softmax streams that ping-pong on the tensor pipe (while one stream's 128 softmax threads
+// work on S, the tensor pipe runs the other stream's P*V and next Q*K^T):
+//   mode A (pair item)  : stream s owns query tile 2*pair+s; both streams walk the same KV tiles, so one K/V fetch
+//                         feeds 256 query rows (halves the L2->SM traffic of 128-row CTAs);
+//   mode B (single item): the group's odd last query tile; stream s walks KV tiles t0+s, t0+s+2, ... -- Split-S inside
+//                         the CTA -- and the two (O, m, l) are merged by log-sum-exp in the epilogue, straight out of
+//                         TMEM (no HBM round trip).
+// Warp roles (416 threads): warps 0-3 softmax stream 0, warps 4-7 softmax stream 1 (thread = query row), warps 8-11
+// producers (16-byte cp.async row gather into 128B-swizzled panels; K and V of a tile share one index computation,
+// indices are prefetched a tile ahead so the gather runs at HBM speed), warp 12 issues every tcgen05.mma (one elected
+// lane, converged warp so the descriptors stay in uniform registers).
+// TMEM (512 columns): S_s at 128*s (P aliases it as packed bf16), O_s at 256 + 128*s.
+// K/V ring: kStages tile slots; tile t of an item occupies loads 2*(t-t0) (K) and 2*(t-t0)+1 (V) counted from the
+// item's first load; a slot is released by a tcgen05.commit after its last user (stream 1 in mode A).
 #include "pdllm_internal.h"
 #include "ptx.cuh"
+
+#ifdef PDLLM_TRACE
+// Perf-debug build only (-DPDLLM_TRACE, never the shipped library): CTA 0 logs (clock64, code, arg) per role.
+__device__ long long *g_pdllm_trace = nullptr;
+extern "C" int pdllm_debug_set_trace(void *dev_buf) {
+    return (int)cudaMemcpyToSymbol(g_pdllm_trace, &dev_buf, sizeof(void *));
+}
+#define PDLLM_TRACE_DECL(role) int tr_n = 0; const int tr_role = (role);
+#define PDLLM_TR(code, arg)                                                                       \
+    do {                                                                                          \
+        if (blockIdx.x == 0 && g_pdllm_trace && tr_n < 4096) {                                    \
+            g_pdllm_trace[(tr_role * 4096 + tr_n) * 2] = clock64();                               \
+            g_pdllm_trace[(tr_role * 4096 + tr_n) * 2 + 1] = ((long long)(code) << 32) | (unsigned)(arg); \
+            ++tr_n;                                                                               \
+        }                                                                                         \
+    } while (0)
+#else
+#define PDLLM_TRACE_DECL(role)
+#define PDLLM_TR(code, arg)
+#endif
 
 namespace pdllm {
 
 namespace {
 
-constexpr int kSoftmaxThreads = 128;
+constexpr int kSoftmaxThreads = 128;                      // per stream
 constexpr int kProducerThreads = 128;
-constexpr int kAttnThreads = kSoftmaxThreads + kProducerThreads + 32;   // + the MMA warp
+constexpr int kProducerWarp0 = 8;
+constexpr int kMmaWarp0 = 12;
+constexpr int kAttnThreads = 2 * kSoftmaxThreads + kProducerThreads + 32;
 constexpr int kInvalidRow = INT32_MIN;
-constexpr float kRescaleThreshold = 8.0f;   // log2 units: P stays <= 2^8 between reference-max updates
+constexpr float kRescaleThreshold = 8.0f;                 // log2 units: P stays <= 2^8 between reference-max updates
+constexpr int kMaxPending = 4;                            // cp.async groups in flight per producer thread
 
 struct AttnParams {
     const uint16_t *Q, *Kc, *Vc, *Kd, *Vd;
     const int32_t *ids, *keep;
     uint16_t *O;
     float *LSE, *O_part, *lse_part;
-    int H_kv, N, Cp, K, Bk, L_s, S_pre, S_kv, rows_g;
-    int n_splits, n_tiles;
-    int64_t total_rows;    // B*H*L
-    float c2;              // scale * log2(e)
+    int N, Cp, K, Bk, L_s, S_pre, S_kv, rows_g;
+    int n_splits, n_tiles;                                // KV tiles of the whole sequence
+    int n_qt, n_pairs, n_single;                          // query tiles per group: n_qt = 2*n_pairs + n_single
+    int n_pair_items, n_items;
+    int64_t total_rows;                                   // B*H*L
+    float c2;                                             // scale * log2(e)
 };
 
-enum { BAR_QFULL = 0, BAR_KFULL, BAR_VFULL, BAR_SREADY, BAR_PREADY, BAR_PVDONE, BAR_COUNT };
+struct Item {
+    int bg, q0, t0, nt, split;
+    bool modeA;
+};
+
+__device__ __forceinline__ Item decode_item(const AttnParams &p, int i) {
+    Item it;
+    if (i < p.n_pair_items) {
+        it.modeA = true;
+        it.split = i % p.n_splits;
+        const int rest = i / p.n_splits;
+        it.q0 = 2 * (rest % p.n_pairs);
+        it.bg = rest / p.n_pairs;
+    } else {
+        i -= p.n_pair_items;
+        it.modeA = false;
+        it.split = i % p.n_splits;
+        it.bg = i / p.n_splits;
+        it.q0 = p.n_qt - 1;
+    }
+    it.t0 = (int)((int64_t)it.split * p.n_tiles / p.n_splits);
+    it.nt = (int)((int64_t)(it.split + 1) * p.n_tiles / p.n_splits) - it.t0;
+    return it;
+}
 
 template <int D>
-__global__ void __launch_bounds__(kAttnThreads, 2) attn_kernel(const AttnParams p) {
-    constexpr int kPanels = D / 64;                 // 64-column (128-byte) panels per row
-    constexpr int kChunksPerRow = D / 8;            // 16-byte chunks per row
-    constexpr int kRowsPerInstr = 32 / kChunksPerRow;
-    constexpr uint32_t kPanelBytes = 128 * 128;     // [128 rows][128 B]
-    constexpr uint32_t kTileBytes = kPanels * kPanelBytes;
-    constexpr uint32_t kTmemCols = 256;             // S/P: 128 columns, O: D columns
-    constexpr uint32_t kOCol = 128;
+struct AttnCfg {
+    static constexpr int kPanels = D / 64;                   // 64-column (128-byte) panels per row
+    static constexpr uint32_t kPanelBytes = 128 * 128;       // [128 rows][128 B]
+    static constexpr uint32_t kTileBytes = kPanels * kPanelBytes;
+    static constexpr int kStages = 5;
+    static constexpr size_t kSmem = 1024 + (size_t)(2 + kStages) * kTileBytes;
+};
+
+// barrier indices (kv_full / kv_free follow)
+enum { BAR_QFULL = 0, BAR_QFREE, BAR_SREADY0, BAR_SREADY1, BAR_PREADY0, BAR_PREADY1, BAR_OREADY0, BAR_OREADY1,
+       BAR_OFREE0, BAR_OFREE1, BAR_KV };
+
+// D[tmem] (+)= A[smem] * B[smem] with the descriptors given as (low word, constant high word)
+__device__ __forceinline__ void umma_ss_lohi(uint32_t d_tmem, uint32_t a_lo, uint32_t b_lo, uint32_t desc_hi, uint32_t idesc,
+                                             uint32_t accumulate) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t.reg .b64 da, db;\n\tsetp.ne.b32 p, %5, 0;\n\t"
+        "mov.b64 da, {%1, %3};\n\tmov.b64 db, {%2, %3};\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], da, db, %4, p;\n\t}"
+        ::"r"(d_tmem), "r"(a_lo), "r"(b_lo), "r"(desc_hi), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
+// D[tmem] (+)= A[tmem] * B[smem]
+__device__ __forceinline__ void umma_ts_lohi(uint32_t d_tmem, uint32_t a_tmem, uint32_t b_lo, uint32_t desc_hi, uint32_t idesc,
+                                             uint32_t accumulate) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t.reg .b64 db;\n\tsetp.ne.b32 p, %5, 0;\n\t"
+        "mov.b64 db, {%2, %3};\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], db, %4, p;\n\t}"
+        ::"r"(d_tmem), "r"(a_tmem), "r"(b_lo), "r"(desc_hi), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
+
+template <int D>
+__global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams p) {
+    using Cfg = AttnCfg<D>;
+    constexpr int ST = Cfg::kStages;
+    constexpr int kChunksPerRow = D / 8;                  // 16-byte chunks per row
+    constexpr int kRowsPerInstr = 32 / kChunksPerRow;     // rows covered by one warp-level cp.async
+    constexpr uint32_t kTmemCols = 512;
+    constexpr uint32_t kOCol = 256;
 
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
-    const uint32_t sQ = smem_base, sK = smem_base + kTileBytes, sV = smem_base + 2 * kTileBytes;
+    auto sQ = [&](int s) { return smem_base + Cfg::kTileBytes * (uint32_t)s; };
+    auto sKV = [&](int slot) { return smem_base + Cfg::kTileBytes * (uint32_t)(2 + slot); };
 
-    __shared__ uint64_t bars[BAR_COUNT];
+    __shared__ uint64_t bars[BAR_KV + 2 * ST];
     __shared__ uint32_t tmem_slot;
-    __shared__ int32_t s_ids[64];
-    __shared__ int32_t s_table[128];
+    __shared__ float s_ml[kSoftmaxThreads][2];            // mode B: stream 1's (m_ref, l) for the in-CTA merge
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const int mt = blockIdx.x, bg = blockIdx.y, split = blockIdx.z;
-    const int t0 = (int)((int64_t)split * p.n_tiles / p.n_splits);
-    const int t1 = (int)((int64_t)(split + 1) * p.n_tiles / p.n_splits);
-    const int nt = t1 - t0;
-
     const uint32_t bar0 = smem_u32(&bars[0]);
     auto bar = [&](int i) { return bar0 + 8u * i; };
+    auto kv_full = [&](int slot) { return bar0 + 8u * (BAR_KV + slot); };
+    auto kv_free = [&](int slot) { return bar0 + 8u * (BAR_KV + ST + slot); };
 
     if (tid == 0) {
         mbar_init(bar(BAR_QFULL), kProducerThreads);
-        mbar_init(bar(BAR_KFULL), kProducerThreads);
-        mbar_init(bar(BAR_VFULL), kProducerThreads);
-        mbar_init(bar(BAR_SREADY), 1);
-        mbar_init(bar(BAR_PREADY), kSoftmaxThreads);
-        mbar_init(bar(BAR_PVDONE), 1);
+        mbar_init(bar(BAR_QFREE), 1);
+        for (int s = 0; s < 2; ++s) {
+            mbar_init(bar(BAR_SREADY0 + s), 1);
+            mbar_init(bar(BAR_PREADY0 + s), kSoftmaxThreads);
+            mbar_init(bar(BAR_OREADY0 + s), 1);
+            mbar_init(bar(BAR_OFREE0 + s), kSoftmaxThreads);
+        }
+        for (int s = 0; s < ST; ++s) {
+            mbar_init(kv_full(s), kProducerThreads);
+            mbar_init(kv_free(s), 1);
+        }
         fence_mbar_init();
     }
-    if (tid < p.K) s_ids[tid] = p.ids[(int64_t)bg * p.K + tid];
-    if (warp == 8) {
+    if (warp == kMmaWarp0) {
         tmem_alloc(smem_u32(&tmem_slot), kTmemCols);
         tmem_relinquish();
     }
@@ -82,244 +173,464 @@ __global__ void __launch_bounds__(kAttnThreads, 2) attn_kernel(const AttnParams 
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem = tmem_slot;
-    const uint32_t tS = tmem, tO = tmem + kOCol;
 
-    if (warp >= 4 && warp < 8) {
-        // =============================== producers: gather ===============================
-        const int pt = tid - kSoftmaxThreads, pw = pt >> 5;
+    if (warp >= kProducerWarp0 && warp < kMmaWarp0) {
+        // =============================== producers: index-driven gather ===============================
+        const int pt = tid - kProducerWarp0 * 32, pw = pt >> 5;
         const int rsub = lane / kChunksPerRow, c = lane % kChunksPerRow;
-        const uint32_t dst_pc = (uint32_t)(c >> 3) * kPanelBytes;
-        const uint16_t *Kc = p.Kc + (int64_t)bg * p.N * p.Cp * D, *Vc = p.Vc + (int64_t)bg * p.N * p.Cp * D;
-        const uint16_t *Kd = p.Kd + (int64_t)bg * p.L_s * D, *Vd = p.Vd + (int64_t)bg * p.L_s * D;
-        {   // Q tile: rows mt*128 .. +127 of the rows_g contiguous rows of this KV group
-            const uint16_t *Qg = p.Q + (int64_t)bg * p.rows_g * D;
-#pragma unroll 4
-            for (int i = 0; i < kChunksPerRow; ++i) {
-                const int r = pw * 32 + i * kRowsPerInstr + rsub;
-                const int qr = mt * kTileM + r;
-                const bool ok = qr < p.rows_g;
-                cp_async16_zfill(sQ + dst_pc + sw128_off(r, c & 7), ok ? Qg + (int64_t)qr * D + c * 8 : Qg, ok ? 16u : 0u);
-            }
-            cp_async_commit();
-            cp_async_wait<0>();
+        const uint32_t dst_pc = (uint32_t)(c >> 3) * Cfg::kPanelBytes;
+        // destination of (row pw*32 + i*RPI + rsub, chunk c) inside a tile: pw*32 is a multiple of 8, so the
+        // 128B-swizzle term (c ^ row) & 7 is x7 ^ (i*RPI & 7) with x7 = (c & 7) ^ rsub
+        const uint32_t dst_thread = dst_pc + (uint32_t)(pw * 32 + rsub) * 128u;
+        const uint32_t x7 = (uint32_t)((c & 7) ^ rsub);
+        uint32_t pend0 = 0, pend1 = 0, pend2 = 0, pend3 = 0;   // barriers of the committed, unpublished groups (oldest first)
+        int np = 0;
+        static_assert(kMaxPending == 4, "the pending list is four registers");
+        auto flush_one = [&]() {                          // oldest group has landed -> publish it
             fence_proxy_async_smem();
-            mbar_arrive(bar(BAR_QFULL));
-        }
-        const int kv_end = min(p.S_kv, t1 * kTileN);
-        for (int jj = 0; jj < nt; ++jj) {
-            const int j = t0 + jj;
-            // row table of this tile (a3): virtual row -> cache row (>= 0) / decode row (< 0)
-            {
-                const int vr = j * kTileN + pt;
+            mbar_arrive(pend0);
+            pend0 = pend1;
+            pend1 = pend2;
+            pend2 = pend3;
+            --np;
+        };
+        auto flush_all = [&]() {
+            cp_async_wait<0>();
+            while (np > 0) flush_one();
+        };
+        auto track = [&](uint32_t b) {                    // the group just committed completes barrier b
+            if (np == 0) pend0 = b;
+            else if (np == 1) pend1 = b;
+            else if (np == 2) pend2 = b;
+            else pend3 = b;
+            if (++np == kMaxPending) {
+                cp_async_wait<kMaxPending - 1>();
+                flush_one();
+            }
+        };
+        // a blocking wait on a consumer-driven barrier never holds back landed loads (so it cannot deadlock)
+        auto wait_free = [&](uint32_t b, uint32_t parity) {
+            if (!mbar_try_wait(b, parity)) {
+                flush_all();
+                mbar_wait(b, parity);
+            }
+        };
+        // the cp.async of this thread for one tile: rows pw*32 + i*RPI + rsub, chunk c; the row addresses live one
+        // per lane (lane = row inside the warp's 32) and are fetched by shuffle; address 0 = zero-fill
+        auto issue_rows = [&](uint32_t dst_tile, uint32_t my_lo, uint32_t my_hi, const void *dummy) {
+#pragma unroll
+            for (int i = 0; i < kChunksPerRow; ++i) {
+                const int rl = i * kRowsPerInstr + rsub;
+                const uint32_t lo = __shfl_sync(0xffffffffu, my_lo, rl), hi = __shfl_sync(0xffffffffu, my_hi, rl);
+                const uint64_t row_addr = ((uint64_t)hi << 32) | lo;
+                const bool ok = row_addr != 0ull;
+                const uint64_t src = ok ? row_addr + (uint64_t)(c * 16) : reinterpret_cast<uint64_t>(dummy);
+                const uint32_t sw = (x7 ^ (uint32_t)((i * kRowsPerInstr) & 7)) << 4;
+                cp_async16_zfill(dst_tile + dst_thread + (uint32_t)(i * kRowsPerInstr) * 128u + sw,
+                                 reinterpret_cast<const void *>(src), ok ? 16u : 0u);
+            }
+        };
+        uint32_t lq = 0;                                  // ring load counter (continues across items)
+        int n_done = 0;                                   // items finished by this CTA
+        PDLLM_TRACE_DECL(0)
+        for (int ii = blockIdx.x; ii < p.n_items; ii += gridDim.x, ++n_done) {
+            const Item it = decode_item(p, ii);
+            const int64_t bg = it.bg;
+            const uint16_t *Kc = p.Kc + bg * p.N * p.Cp * D, *Vc = p.Vc + bg * p.N * p.Cp * D;
+            const uint16_t *Kd = p.Kd + bg * p.L_s * D, *Vd = p.Vd + bg * p.L_s * D;
+            const int32_t *keep = p.keep ? p.keep + bg * p.N * p.Bk : nullptr;
+            // the group's K <= 64 chunk ids live in two registers per lane (lane l: ids[l], ids[l + 32])
+            const int ids_lo = lane < p.K ? __ldg(p.ids + bg * p.K + lane) : 0;
+            const int ids_hi = lane + 32 < p.K ? __ldg(p.ids + bg * p.K + lane + 32) : 0;
+            // a3: virtual row -> cache row (>= 0) / decode row (< 0) / invalid; one row per producer thread
+            auto row_index = [&](int tile) {
+                const int vr = tile * kTileN + pt;
+                const bool pre = vr < p.S_pre;
+                const int k = pre ? vr / p.Bk : 0, t = vr - k * p.Bk;
+                const int n_lo = __shfl_sync(0xffffffffu, ids_lo, k & 31), n_hi = __shfl_sync(0xffffffffu, ids_hi, k & 31);
+                const int n = k < 32 ? n_lo : n_hi;
                 int idx = kInvalidRow;
-                if (vr < kv_end) {
-                    if (vr < p.S_pre) {
-                        const int k = vr / p.Bk, t = vr - k * p.Bk;
-                        const int n = s_ids[k];
-                        const int slot = p.keep ? __ldg(p.keep + ((int64_t)bg * p.N + n) * p.Bk + t) : t;
-                        idx = n * p.Cp + slot;
-                    } else {
-                        idx = -(vr - p.S_pre) - 1;
+                if (pre) idx = n * p.Cp + (keep ? __ldg(keep + (int64_t)n * p.Bk + t) : t);
+                else if (vr < p.S_kv) idx = -(vr - p.S_pre) - 1;
+                return idx;
+            };
+            int idx_next = row_index(it.t0);
+            for (int jt = 0; jt < it.nt; ++jt, lq += 2) {
+                const int my_idx = idx_next;
+                if (pt == 0) PDLLM_TR(10, lq);
+                if (jt + 1 < it.nt) idx_next = row_index(it.t0 + jt + 1);   // in flight while this tile is issued
+                const int slot_k = (int)(lq % ST), slot_v = (int)((lq + 1) % ST);
+                if (lq >= (uint32_t)ST) wait_free(kv_free(slot_k), ((lq / ST) - 1) & 1u);
+                if (lq + 1 >= (uint32_t)ST) wait_free(kv_free(slot_v), (((lq + 1) / ST) - 1) & 1u);
+                if (pt == 0) PDLLM_TR(11, lq);
+                // this thread's row (pw*32 + lane) as global byte addresses in K and V; 0 = beyond the sequence
+                const bool in_cache = my_idx >= 0;
+                const int64_t row_off = in_cache ? (int64_t)my_idx * D : (int64_t)(-my_idx - 1) * D;
+                const bool valid = my_idx != kInvalidRow;
+                const uint64_t ka = valid ? reinterpret_cast<uint64_t>((in_cache ? Kc : Kd) + row_off) : 0ull;
+                const uint64_t va = valid ? reinterpret_cast<uint64_t>((in_cache ? Vc : Vd) + row_off) : 0ull;
+                issue_rows(sKV(slot_k), (uint32_t)ka, (uint32_t)(ka >> 32), Kc);
+                cp_async_commit();
+                track(kv_full(slot_k));
+                issue_rows(sKV(slot_v), (uint32_t)va, (uint32_t)(va >> 32), Vc);
+                cp_async_commit();
+                if (pt == 0) PDLLM_TR(12, lq);
+                track(kv_full(slot_v));
+                if (pt == 0) PDLLM_TR(13, np);
+                if (jt == 0) {
+                    // the item's Q tile(s), once the previous item's Q*K^T are all done
+                    if (n_done > 0) wait_free(bar(BAR_QFREE), (uint32_t)(n_done - 1) & 1u);
+                    const uint16_t *Qg = p.Q + bg * p.rows_g * D;
+                    const int n_q = it.modeA ? 2 : 1;
+                    for (int s = 0; s < n_q; ++s) {
+#pragma unroll
+                        for (int i = 0; i < kChunksPerRow; ++i) {
+                            const int r = pw * 32 + i * kRowsPerInstr + rsub;
+                            const int qr = (it.q0 + s) * kTileM + r;
+                            const bool ok = qr < p.rows_g;
+                            const uint32_t sw = (x7 ^ (uint32_t)((i * kRowsPerInstr) & 7)) << 4;
+                            cp_async16_zfill(sQ(s) + dst_thread + (uint32_t)(i * kRowsPerInstr) * 128u + sw,
+                                             ok ? Qg + (int64_t)qr * D + c * 8 : Qg, ok ? 16u : 0u);
+                        }
                     }
-                }
-                s_table[pt] = idx;
-            }
-            asm volatile("bar.sync 1, 128;" ::: "memory");
-            const int n_valid = min(kTileN, kv_end - j * kTileN);
-            const int n_mma = (n_valid + 15) & ~15;
-            if (jj > 0) mbar_wait(bar(BAR_SREADY), (jj - 1) & 1);      // QK(j-1) done: K buffer free
-#pragma unroll 4
-            for (int i = 0; i < kChunksPerRow; ++i) {
-                const int r = pw * 32 + i * kRowsPerInstr + rsub;
-                if (r < n_mma) {
-                    const int idx = s_table[r];
-                    const bool ok = idx != kInvalidRow;
-                    const uint16_t *src = idx >= 0 ? Kc + (int64_t)idx * D : Kd + (int64_t)(-idx - 1) * D;
-                    cp_async16_zfill(sK + dst_pc + sw128_off(r, c & 7), ok ? src + c * 8 : Kc, ok ? 16u : 0u);
+                    cp_async_commit();
+                    track(bar(BAR_QFULL));
                 }
             }
-            cp_async_commit();
-            if (jj > 0) mbar_wait(bar(BAR_PVDONE), (jj - 1) & 1);      // PV(j-1) done: V buffer free
-#pragma unroll 4
-            for (int i = 0; i < kChunksPerRow; ++i) {
-                const int r = pw * 32 + i * kRowsPerInstr + rsub;
-                if (r < n_mma) {
-                    const int idx = s_table[r];
-                    const bool ok = idx != kInvalidRow;
-                    const uint16_t *src = idx >= 0 ? Vc + (int64_t)idx * D : Vd + (int64_t)(-idx - 1) * D;
-                    cp_async16_zfill(sV + dst_pc + sw128_off(r, c & 7), ok ? src + c * 8 : Vc, ok ? 16u : 0u);
-                }
-            }
-            cp_async_commit();
-            cp_async_wait<1>();
-            fence_proxy_async_smem();
-            mbar_arrive(bar(BAR_KFULL));
-            cp_async_wait<0>();
-            fence_proxy_async_smem();
-            mbar_arrive(bar(BAR_VFULL));
-            asm volatile("bar.sync 1, 128;" ::: "memory");              // table may be rewritten
         }
-    } else if (warp == 8) {
+        flush_all();
+    } else if (warp == kMmaWarp0) {
         // =============================== MMA issuer ===============================
-        if (lane == 0) {
-            const int kv_end = min(p.S_kv, t1 * kTileN);
-            mbar_wait(bar(BAR_QFULL), 0);
-            for (int jj = 0; jj < nt; ++jj) {
-                const int j = t0 + jj;
-                const int n_valid = min(kTileN, kv_end - j * kTileN);
-                const uint32_t n_mma = (uint32_t)(n_valid + 15) & ~15u;
-                mbar_wait(bar(BAR_KFULL), jj & 1);
-                if (jj > 0) mbar_wait(bar(BAR_PVDONE), (jj - 1) & 1);  // S aliases P(j-1)
+        // One warp issues both streams' MMAs in the fixed order QK(0,0) QK(1,0) { PV(0,j) QK(0,j+1) PV(1,j) QK(1,j+1) }:
+        // the in-order tensor pipe then keeps the two softmax streams in anti-phase (one stream's exponentials run
+        // under the other stream's MMAs).  The warp stays converged (all lanes wait on the barriers); one elected
+        // lane issues the tcgen05 instructions, so the descriptors stay in uniform registers.
+        PDLLM_TRACE_DECL(1)
+        uint32_t lq_base = 0;
+        uint32_t n_pready[2] = {0, 0}, n_oready[2] = {0, 0};
+        int n_done = 0;
+        constexpr uint32_t idesc_pv = umma_idesc_bf16(kTileM, D, 0, 1);
+        // descriptor words: K-major operands (Q, K): lbo 16, sbo 1024; MN-major V: lbo = panel stride, sbo 1024
+        const uint32_t hi_k = (uint32_t)(umma_desc_sw128(0, 16, 1024) >> 32);
+        const uint32_t hi_v = (uint32_t)(umma_desc_sw128(0, Cfg::kPanelBytes, 1024) >> 32);
+        const uint32_t lo_k = (uint32_t)umma_desc_sw128(0, 16, 1024), lo_v = (uint32_t)umma_desc_sw128(0, Cfg::kPanelBytes, 1024);
+        for (int ii = blockIdx.x; ii < p.n_items; ii += gridDim.x, ++n_done) {
+            const Item it = decode_item(p, ii);
+            const int n_s[2] = {it.modeA ? it.nt : (it.nt + 1) / 2, it.modeA ? it.nt : it.nt / 2};
+            const int qk_total = n_s[0] + n_s[1];
+            int qk_issued = 0;
+            auto tile_of = [&](int s, int j) { return it.modeA ? it.t0 + j : it.t0 + 2 * j + s; };
+            auto n_mma_of = [&](int tile) { return (uint32_t)((min(kTileN, p.S_kv - tile * kTileN) + 15) & ~15); };
+            auto issue_qk = [&](int s, int j) {
+                const int tile = tile_of(s, j);
+                const uint32_t q = lq_base + 2u * (uint32_t)(tile - it.t0);
+                const int slot = (int)(q % ST);
+                const bool release = !it.modeA || s == 1;     // last user of this K tile
+                if (lane == 0) PDLLM_TR(20, s);
+                if (!it.modeA || s == 0) mbar_wait(kv_full(slot), (q / ST) & 1u);
                 tc_fence_after();
-                const uint32_t idesc_qk = umma_idesc_bf16(kTileM, n_mma, 0, 0);
+                const bool last_qk = ++qk_issued == qk_total;
+                if (elect_one()) {
+                    const uint32_t a_lo = lo_k | ((sQ(it.modeA ? s : 0) & 0x3FFFFu) >> 4);
+                    const uint32_t b_lo = lo_k | ((sKV(slot) & 0x3FFFFu) >> 4);
+                    const uint32_t idesc = umma_idesc_bf16(kTileM, n_mma_of(tile), 0, 0);
+                    const uint32_t tS = tmem + 128u * s;
 #pragma unroll
-                for (int ks = 0; ks < D / 16; ++ks) {
-                    const uint32_t off = (uint32_t)(ks >> 2) * kPanelBytes + (uint32_t)(ks & 3) * 32u;
-                    umma_ss(tS, umma_desc_sw128(sQ + off, 16, 1024), umma_desc_sw128(sK + off, 16, 1024), idesc_qk, ks > 0);
-                }
-                umma_commit(bar(BAR_SREADY));
-                mbar_wait(bar(BAR_PREADY), jj & 1);
-                mbar_wait(bar(BAR_VFULL), jj & 1);
-                tc_fence_after();
-                const uint32_t idesc_pv = umma_idesc_bf16(kTileM, D, 0, 1);
-                const int ksteps = (int)(n_mma >> 4);
-                for (int ks = 0; ks < ksteps; ++ks) {
-                    // 16 kv rows per step: A = 8 TMEM columns of packed bf16 P, B = V rows (MN-major)
-                    umma_ts(tO, tS + 8u * ks, umma_desc_sw128(sV + 2048u * ks, kPanelBytes, 1024), idesc_pv,
-                            (jj > 0 || ks > 0) ? 1u : 0u);
-                }
-                umma_commit(bar(BAR_PVDONE));
-            }
-        }
-        __syncwarp();
-    } else {
-        // =============================== softmax (thread = row) ===============================
-        const uint32_t lane_base = (uint32_t)(warp * 32) << 16;
-        const int kv_end = min(p.S_kv, t1 * kTileN);
-        float m_ref = -INFINITY, l = 0.f;
-        for (int jj = 0; jj < nt; ++jj) {
-            const int j = t0 + jj;
-            const int n_valid = min(kTileN, kv_end - j * kTileN);
-            const int n_mma = (n_valid + 15) & ~15;
-            const int nchunks = (n_mma + 31) >> 5;
-            mbar_wait(bar(BAR_SREADY), jj & 1);
-            tc_fence_after();
-            // pass 1: row max of the raw logits
-            float tmax = -INFINITY;
-            for (int ch = 0; ch < nchunks; ++ch) {
-                uint32_t v[32];
-                tmem_ld32(tS + lane_base + 32u * ch, v);
-                tmem_wait_ld();
-                if (n_valid == kTileN) {
-#pragma unroll
-                    for (int e = 0; e < 32; ++e) tmax = fmaxf(tmax, __uint_as_float(v[e]));
-                } else {
-#pragma unroll
-                    for (int e = 0; e < 32; ++e)
-                        if (ch * 32 + e < n_valid) tmax = fmaxf(tmax, __uint_as_float(v[e]));
-                }
-            }
-            const float tm2 = tmax * p.c2;
-            const bool need = tm2 > m_ref + kRescaleThreshold;          // always true on the first tile
-            if (__any_sync(0xffffffffu, need)) {
-                const float m_new = need ? tm2 : m_ref;
-                const float f = need ? ex2_approx(m_ref - m_new) : 1.f;  // m_ref = -inf -> 0
-                l *= f;
-                if (jj > 0) {
-#pragma unroll 1
-                    for (int ch = 0; ch < D / 32; ++ch) {
-                        uint32_t o[32];
-                        tmem_ld32(tO + lane_base + 32u * ch, o);
-                        tmem_wait_ld();
-#pragma unroll
-                        for (int e = 0; e < 32; ++e) o[e] = __float_as_uint(__uint_as_float(o[e]) * f);
-                        tmem_st32(tO + lane_base + 32u * ch, o);
+                    for (int ks = 0; ks < D / 16; ++ks) {
+                        // 16 columns = 32 bytes inside the 128-byte swizzle row; next panel every 4 steps
+                        const uint32_t koff = (uint32_t)(((ks >> 2) * Cfg::kPanelBytes + (ks & 3) * 32u) >> 4);
+                        umma_ss_lohi(tS, a_lo + koff, b_lo + koff, hi_k, idesc, ks > 0);
                     }
+                    umma_commit(bar(BAR_SREADY0 + s));
+                    if (release) umma_commit(kv_free(slot));
+                    if (last_qk) umma_commit(bar(BAR_QFREE));
                 }
-                m_ref = m_new;
+                __syncwarp();
+                if (lane == 0) PDLLM_TR(22, s);
+            };
+            mbar_wait(bar(BAR_QFULL), (uint32_t)n_done & 1u);
+            issue_qk(0, 0);
+            if (n_s[1] > 0) issue_qk(1, 0);
+            for (int j = 0; j < n_s[0]; ++j) {
+                for (int s = 0; s < 2; ++s) {
+                    if (j >= n_s[s]) continue;
+                    const int tile = tile_of(s, j);
+                    const uint32_t q = lq_base + 2u * (uint32_t)(tile - it.t0) + 1u;
+                    const int slot = (int)(q % ST);
+                    const bool release = !it.modeA || s == 1;     // last user of this V tile
+                    if (lane == 0) PDLLM_TR(23, s);
+                    mbar_wait(bar(BAR_PREADY0 + s), n_pready[s]++ & 1u);
+                    if (lane == 0) PDLLM_TR(24, s);
+                    if (j == 0 && n_oready[s] > 0) mbar_wait(bar(BAR_OFREE0 + s), (n_oready[s] - 1) & 1u);
+                    if (!it.modeA || s == 0) mbar_wait(kv_full(slot), (q / ST) & 1u);
+                    tc_fence_after();
+                    if (lane == 0) PDLLM_TR(25, s);
+                    const int ksteps = (int)(n_mma_of(tile) >> 4);
+                    const bool last_pv = j == n_s[s] - 1;
+                    if (elect_one()) {
+                        // 16 kv rows per step: A = 8 TMEM columns of packed bf16 P, B = 16 V rows (MN-major, 2048 B)
+                        const uint32_t v_lo = lo_v | ((sKV(slot) & 0x3FFFFu) >> 4);
+                        const uint32_t tS = tmem + 128u * s, tO = tmem + kOCol + 128u * s;
+                        if (ksteps == kTileN / 16) {
+#pragma unroll
+                            for (int ks = 0; ks < kTileN / 16; ++ks)
+                                umma_ts_lohi(tO, tS + 8u * ks, v_lo + 128u * ks, hi_v, idesc_pv, (j > 0 || ks > 0) ? 1u : 0u);
+                        } else {
+                            for (int ks = 0; ks < ksteps; ++ks)
+                                umma_ts_lohi(tO, tS + 8u * ks, v_lo + 128u * ks, hi_v, idesc_pv, (j > 0 || ks > 0) ? 1u : 0u);
+                        }
+                        if (release) umma_commit(kv_free(slot));
+                        if (last_pv) umma_commit(bar(BAR_OREADY0 + s));
+                    }
+                    __syncwarp();
+                    if (last_pv) ++n_oready[s];
+                    if (lane == 0) PDLLM_TR(26, s);
+                    if (j + 1 < n_s[s]) issue_qk(s, j + 1);
+                }
             }
-            // pass 2: P = 2^(c2*S - m_ref), packed bf16 into the first 64 columns of S
-            for (int ch = 0; ch < nchunks; ++ch) {
-                uint32_t v[32];
-                tmem_ld32(tS + lane_base + 32u * ch, v);
-                tmem_wait_ld();
-                uint32_t w[16];
-                float lsum = 0.f;
+            lq_base += 2u * it.nt;
+        }
+    } else {
+        // =============================== softmax streams (thread = query row) ===============================
+        const int s = warp >> 2;                          // stream
+        const int row = tid & (kSoftmaxThreads - 1);
+        const uint32_t lane_base = (uint32_t)((warp & 3) * 32) << 16;
+        const uint32_t tS = tmem + 128u * s + lane_base, tO = tmem + kOCol + 128u * s + lane_base;
+        uint32_t n_sready = 0, n_oready = 0;
+        int n_modeB = 0;
+        PDLLM_TRACE_DECL(2 + s)
+        for (int ii = blockIdx.x; ii < p.n_items; ii += gridDim.x) {
+            const Item it = decode_item(p, ii);
+            const int n_mine = it.modeA ? it.nt : (s == 0 ? (it.nt + 1) / 2 : it.nt / 2);
+            float m_ref = -INFINITY, l = 0.f;
+            // multiply the O accumulator of this row by f (PV(s, j-1) completed before S(s, j) was committed)
+            auto scale_O = [&](float f) {
+#pragma unroll 1
+                for (int ch = 0; ch < D / 32; ++ch) {
+                    uint32_t o[32];
+                    tmem_ld32(tO + 32u * ch, o);
+                    tmem_wait_ld();
+#pragma unroll
+                    for (int e = 0; e < 32; ++e) o[e] = __float_as_uint(__uint_as_float(o[e]) * f);
+                    tmem_st32(tO + 32u * ch, o);
+                }
+            };
+            // one 32-column chunk of a FULL tile: P = 2^(c2*S - m_ref) as packed bf16, row sum, raw max
+            auto chunk_exp = [&](const uint32_t(&v)[32], uint32_t(&w)[16], float &csum, float &cmax) {
+                float ls[4] = {0.f, 0.f, 0.f, 0.f}, mx[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
 #pragma unroll
                 for (int e = 0; e < 32; e += 2) {
-                    float p0 = ex2_approx(fmaf(__uint_as_float(v[e]), p.c2, -m_ref));
-                    float p1 = ex2_approx(fmaf(__uint_as_float(v[e + 1]), p.c2, -m_ref));
-                    if (n_valid != kTileN) {
-                        if (ch * 32 + e >= n_valid) p0 = 0.f;
-                        if (ch * 32 + e + 1 >= n_valid) p1 = 0.f;
-                    }
-                    lsum += p0 + p1;
+                    const float x0 = __uint_as_float(v[e]), x1 = __uint_as_float(v[e + 1]);
+                    const float p0 = ex2_approx(fmaf(x0, p.c2, -m_ref)), p1 = ex2_approx(fmaf(x1, p.c2, -m_ref));
+                    mx[(e >> 1) & 3] = fmaxf(mx[(e >> 1) & 3], fmaxf(x0, x1));
+                    ls[(e >> 1) & 3] += p0 + p1;
                     w[e >> 1] = pack_bf16x2(p0, p1);
                 }
-                l += lsum;
-                tmem_st16(tS + lane_base + 16u * ch, w);
-            }
-            tmem_wait_st();
-            tc_fence_before();
-            mbar_arrive(bar(BAR_PREADY));
-        }
-        // ------------------------------- epilogue -------------------------------
-        mbar_wait(bar(BAR_PVDONE), (nt - 1) & 1);
-        tc_fence_after();
-        const int qr = mt * kTileM + tid;
-        const bool row_ok = qr < p.rows_g;
-        const int64_t grow = (int64_t)bg * p.rows_g + qr;
-        const float inv = 1.f / l;
-        const float lse = (m_ref + lg2_approx(l)) * 0.6931471805599453f;
-        if (p.n_splits == 1) {
-            if (row_ok) p.LSE[grow] = lse;
-#pragma unroll 1
-            for (int ch = 0; ch < D / 32; ++ch) {
-                uint32_t o[32];
-                tmem_ld32(tO + lane_base + 32u * ch, o);
-                tmem_wait_ld();
-                if (row_ok) {
-                    uint4 *dst = reinterpret_cast<uint4 *>(p.O + grow * D + ch * 32);
+                csum = (ls[0] + ls[1]) + (ls[2] + ls[3]);
+                cmax = fmaxf(fmaxf(mx[0], mx[1]), fmaxf(mx[2], mx[3]));
+            };
+            for (int j = 0; j < n_mine; ++j) {
+                const int tile = it.modeA ? it.t0 + j : it.t0 + 2 * j + s;
+                const int n_valid = min(kTileN, p.S_kv - tile * kTileN);
+                if (row == 0) PDLLM_TR(30, j);
+                mbar_wait(bar(BAR_SREADY0 + s), n_sready++ & 1u);
+                tc_fence_after();
+                if (row == 0) PDLLM_TR(31, j);
+                if (n_valid == kTileN && j > 0) {
+                    // Single pass with the current reference max, TMEM loads one chunk ahead of the arithmetic.  A
+                    // chunk whose max outgrew the reference (rare) raises it by a whole number of octaves BEFORE its P is
+                    // stored: l, O and the P chunks already stored are rescaled by an exact power of two.
+                    float lsum = 0.f;
+                    uint32_t va[32], vb[32];
+                    auto do_chunk = [&](const uint32_t(&v)[32], int ch) {
+                        uint32_t w[16];
+                        float csum, cmax;
+                        chunk_exp(v, w, csum, cmax);
+                        const float over = cmax * p.c2 - m_ref;
+                        if (__any_sync(0xffffffffu, over > kRescaleThreshold)) {
+                            const float up = over > kRescaleThreshold ? ceilf(over) : 0.f;
+                            const float f = ex2_approx(-up);      // exact power of two (1 for rows that are fine)
+                            l *= f;
+                            lsum *= f;
+                            tmem_wait_st();
+                            scale_O(f);
+                            for (int c0 = 0; c0 < ch; ++c0) {     // P chunks of this tile stored so far
+                                uint32_t pw16[16];
+                                tmem_ld16(tS + 16u * c0, pw16);
+                                tmem_wait_ld();
 #pragma unroll
-                    for (int q4 = 0; q4 < 4; ++q4) {
-                        uint4 u;
-                        u.x = pack_bf16x2(__uint_as_float(o[q4 * 8 + 0]) * inv, __uint_as_float(o[q4 * 8 + 1]) * inv);
-                        u.y = pack_bf16x2(__uint_as_float(o[q4 * 8 + 2]) * inv, __uint_as_float(o[q4 * 8 + 3]) * inv);
-                        u.z = pack_bf16x2(__uint_as_float(o[q4 * 8 + 4]) * inv, __uint_as_float(o[q4 * 8 + 5]) * inv);
-                        u.w = pack_bf16x2(__uint_as_float(o[q4 * 8 + 6]) * inv, __uint_as_float(o[q4 * 8 + 7]) * inv);
-                        dst[q4] = u;
+                                for (int e = 0; e < 16; ++e) {
+                                    const float lo = __uint_as_float(pw16[e] << 16) * f, hi = __uint_as_float(pw16[e] & 0xffff0000u) * f;
+                                    pw16[e] = pack_bf16x2(lo, hi);
+                                }
+                                tmem_st16(tS + 16u * c0, pw16);
+                            }
+                            m_ref += up;
+                            chunk_exp(v, w, csum, cmax);
+                        }
+                        lsum += csum;
+                        tmem_st16(tS + 16u * ch, w);
+                    };
+                    tmem_ld32(tS, va);
+                    tmem_wait_ld();
+                    tmem_ld32(tS + 32u, vb);
+                    do_chunk(va, 0);
+                    tmem_wait_ld();
+                    tmem_ld32(tS + 64u, va);
+                    do_chunk(vb, 1);
+                    tmem_wait_ld();
+                    tmem_ld32(tS + 96u, vb);
+                    do_chunk(va, 2);
+                    tmem_wait_ld();
+                    do_chunk(vb, 3);
+                    l += lsum;
+                } else {
+                    // first tile of the stream or a ragged tail tile: max pass, then exp pass with column masks
+                    const int n_mma = (n_valid + 15) & ~15;
+                    const int nchunks = (n_mma + 31) >> 5;
+                    float tmax = -INFINITY;
+                    for (int ch = 0; ch < nchunks; ++ch) {
+                        uint32_t v[32];
+                        tmem_ld32(tS + 32u * ch, v);
+                        tmem_wait_ld();
+                        float mx[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
+#pragma unroll
+                        for (int e = 0; e < 32; ++e)
+                            if (ch * 32 + e < n_valid) mx[e & 3] = fmaxf(mx[e & 3], __uint_as_float(v[e]));
+                        tmax = fmaxf(tmax, fmaxf(fmaxf(mx[0], mx[1]), fmaxf(mx[2], mx[3])));
+                    }
+                    const float tm2 = tmax * p.c2;
+                    const bool need = tm2 > m_ref + kRescaleThreshold;     // always true on the first tile
+                    if (__any_sync(0xffffffffu, need)) {
+                        const float m_new = need ? tm2 : m_ref;
+                        const float f = need ? ex2_approx(m_ref - m_new) : 1.f;   // m_ref = -inf -> 0
+                        l *= f;
+                        if (j > 0) scale_O(f);
+                        m_ref = m_new;
+                    }
+                    for (int ch = 0; ch < nchunks; ++ch) {
+                        uint32_t v[32];
+                        tmem_ld32(tS + 32u * ch, v);
+                        tmem_wait_ld();
+                        uint32_t w[16];
+                        float ls[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+                        for (int e = 0; e < 32; e += 2) {
+                            float p0 = ex2_approx(fmaf(__uint_as_float(v[e]), p.c2, -m_ref));
+                            float p1 = ex2_approx(fmaf(__uint_as_float(v[e + 1]), p.c2, -m_ref));
+                            if (ch * 32 + e >= n_valid) p0 = 0.f;
+                            if (ch * 32 + e + 1 >= n_valid) p1 = 0.f;
+                            ls[(e >> 1) & 3] += p0 + p1;
+                            w[e >> 1] = pack_bf16x2(p0, p1);
+                        }
+                        l += (ls[0] + ls[1]) + (ls[2] + ls[3]);
+                        tmem_st16(tS + 16u * ch, w);
+                    }
+                }
+                tmem_wait_st();
+                tc_fence_before();
+                mbar_arrive(bar(BAR_PREADY0 + s));
+                if (row == 0) PDLLM_TR(33, j);
+            }
+            if (row == 0) PDLLM_TR(34, n_mine);
+            // ------------------------------- epilogue -------------------------------
+            const int qt = it.modeA ? it.q0 + s : it.q0;
+            const int qr = qt * kTileM + row;
+            const bool row_ok = qr < p.rows_g;
+            const int64_t grow = (int64_t)it.bg * p.rows_g + qr;
+            if (n_mine > 0) {
+                mbar_wait(bar(BAR_OREADY0 + s), n_oready++ & 1u);
+                tc_fence_after();
+            }
+            float a_self = 1.f, a_other = 0.f, l_tot = l, m_tot = m_ref;
+            const bool merge_other = !it.modeA && it.nt > 1;    // stream 1 had tiles (uniform per item)
+            if (!it.modeA) {
+                // a5 inside the CTA: stream 1 publishes (m, l); stream 0 merges both accumulators out of TMEM
+                if (s == 1) {
+                    // stream 0 has read the previous single item's pair (named barrier 3: it arrives, we wait)
+                    if (n_modeB > 0) asm volatile("bar.sync 3, 256;" ::: "memory");
+                    s_ml[row][0] = m_ref;
+                    s_ml[row][1] = l;
+                }
+                ++n_modeB;
+                tc_fence_before();
+                asm volatile("bar.sync 2, 256;" ::: "memory");
+                tc_fence_after();
+                if (s == 0) {
+                    const float m1 = s_ml[row][0], l1 = s_ml[row][1];
+                    asm volatile("bar.arrive 3, 256;" ::: "memory");
+                    if (merge_other) {
+                        m_tot = fmaxf(m_ref, m1);
+                        a_self = ex2_approx(m_ref - m_tot);
+                        a_other = ex2_approx(m1 - m_tot);
+                        l_tot = l * a_self + l1 * a_other;
                     }
                 }
             }
-        } else {
-            if (row_ok) p.lse_part[(int64_t)split * p.total_rows + grow] = lse;
-#pragma unroll 1
-            for (int ch = 0; ch < D / 32; ++ch) {
-                uint32_t o[32];
-                tmem_ld32(tO + lane_base + 32u * ch, o);
-                tmem_wait_ld();
-                if (row_ok) {
-                    float4 *dst = reinterpret_cast<float4 *>(p.O_part + ((int64_t)split * p.total_rows + grow) * D + ch * 32);
-#pragma unroll
-                    for (int q4 = 0; q4 < 8; ++q4)
-                        dst[q4] = make_float4(__uint_as_float(o[q4 * 4 + 0]) * inv, __uint_as_float(o[q4 * 4 + 1]) * inv,
-                                              __uint_as_float(o[q4 * 4 + 2]) * inv, __uint_as_float(o[q4 * 4 + 3]) * inv);
+            if (it.modeA || s == 0) {
+                const float inv = 1.f / l_tot;
+                const float lse = (m_tot + lg2_approx(l_tot)) * 0.6931471805599453f;
+                const float w_self = a_self * inv, w_other = a_other * inv;
+                const uint32_t tO_other = tmem + kOCol + 128u + lane_base;    // stream 1's accumulator, same rows
+                if (p.n_splits == 1) {
+                    if (row_ok) p.LSE[grow] = lse;
+                } else {
+                    if (row_ok) p.lse_part[(int64_t)it.split * p.total_rows + grow] = lse;
                 }
+#pragma unroll 1
+                for (int ch = 0; ch < D / 32; ++ch) {
+                    uint32_t o[32];
+                    tmem_ld32(tO + 32u * ch, o);
+                    tmem_wait_ld();
+                    float f[32];
+#pragma unroll
+                    for (int e = 0; e < 32; ++e) f[e] = __uint_as_float(o[e]) * w_self;
+                    if (merge_other) {
+                        tmem_ld32(tO_other + 32u * ch, o);
+                        tmem_wait_ld();
+#pragma unroll
+                        for (int e = 0; e < 32; ++e) f[e] = fmaf(__uint_as_float(o[e]), w_other, f[e]);
+                    }
+                    if (row_ok) {
+                        if (p.n_splits == 1) {
+                            uint4 *dst = reinterpret_cast<uint4 *>(p.O + grow * D + ch * 32);
+#pragma unroll
+                            for (int q4 = 0; q4 < 4; ++q4) {
+                                uint4 u;
+                                u.x = pack_bf16x2(f[q4 * 8 + 0], f[q4 * 8 + 1]);
+                                u.y = pack_bf16x2(f[q4 * 8 + 2], f[q4 * 8 + 3]);
+                                u.z = pack_bf16x2(f[q4 * 8 + 4], f[q4 * 8 + 5]);
+                                u.w = pack_bf16x2(f[q4 * 8 + 6], f[q4 * 8 + 7]);
+                                dst[q4] = u;
+                            }
+                        } else {
+                            float4 *dst =
+                                reinterpret_cast<float4 *>(p.O_part + ((int64_t)it.split * p.total_rows + grow) * D + ch * 32);
+#pragma unroll
+                            for (int q4 = 0; q4 < 8; ++q4)
+                                dst[q4] = make_float4(f[q4 * 4 + 0], f[q4 * 4 + 1], f[q4 * 4 + 2], f[q4 * 4 + 3]);
+                        }
+                    }
+                }
+                tc_fence_before();
+                mbar_arrive(bar(BAR_OFREE0 + s));
+                if (merge_other) mbar_arrive(bar(BAR_OFREE1));      // stream 0 has drained stream 1's accumulator
             }
+            if (row == 0) PDLLM_TR(35, n_mine);
         }
     }
     tc_fence_before();
     __syncthreads();
-    if (warp == 8) tmem_dealloc(tmem, kTmemCols);
+    if (warp == kMmaWarp0) tmem_dealloc(tmem, kTmemCols);
 }
 
 template <int D>
-cudaError_t launch_attn_d(const AttnParams &p, int m_tiles, int BG, cudaStream_t st) {
-    constexpr size_t smem = 1024 + 3 * (size_t)(D / 64) * 128 * 128;
-    cudaError_t e = cudaFuncSetAttribute(attn_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+cudaError_t launch_attn_d(const AttnParams &p, cudaStream_t st) {
+    using Cfg = AttnCfg<D>;
+    cudaError_t e = cudaFuncSetAttribute(attn_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::kSmem);
     if (e != cudaSuccess) return e;
-    dim3 grid((unsigned)m_tiles, (unsigned)BG, (unsigned)p.n_splits);
-    attn_kernel<D><<<grid, kAttnThreads, smem, st>>>(p);
+    const int grid = p.n_items < device_num_sms() ? p.n_items : device_num_sms();
+    attn_kernel<D><<<grid, kAttnThreads, Cfg::kSmem, st>>>(p);
     return cudaGetLastError();
 }
 
@@ -340,15 +651,19 @@ cudaError_t launch_attn(const Dims &s, const void *Q_dec, const void *Kcache, co
     p.LSE = LSE;
     p.O_part = O_part;
     p.lse_part = lse_part;
-    p.H_kv = s.H_kv; p.N = s.N; p.Cp = s.Cp; p.K = s.K; p.Bk = s.Bk; p.L_s = s.L_s;
+    p.N = s.N; p.Cp = s.Cp; p.K = s.K; p.Bk = s.Bk; p.L_s = s.L_s;
     p.S_pre = s.S_pre; p.S_kv = s.S_kv; p.rows_g = s.rows_g;
     p.n_tiles = (s.S_kv + kTileN - 1) / kTileN;
     p.n_splits = n_splits;
+    p.n_qt = (s.rows_g + kTileM - 1) / kTileM;
+    p.n_pairs = p.n_qt / 2;
+    p.n_single = p.n_qt & 1;
+    const int BG = s.B * s.H_kv;
+    p.n_pair_items = BG * p.n_pairs * n_splits;
+    p.n_items = p.n_pair_items + BG * p.n_single * n_splits;
     p.total_rows = (int64_t)s.B * s.H * s.L;
     p.c2 = s.scale * 1.4426950408889634f;
-    const int m_tiles = (s.rows_g + kTileM - 1) / kTileM;
-    const int BG = s.B * s.H_kv;
-    return s.d == 128 ? launch_attn_d<128>(p, m_tiles, BG, st) : launch_attn_d<64>(p, m_tiles, BG, st);
+    return s.d == 128 ? launch_attn_d<128>(p, st) : launch_attn_d<64>(p, st);
 }
 
 }  // namespace pdllm

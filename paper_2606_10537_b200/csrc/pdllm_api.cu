@@ -48,15 +48,45 @@ int resolve(const pdllm_shape *sh, bool has_keep, Dims *out) {
 }
 
 int kv_tiles(const Dims &d) { return (d.S_kv + kTileN - 1) / kTileN; }
-int m_tiles(const Dims &d) { return d.B * d.H_kv * ((d.rows_g + kTileM - 1) / kTileM); }
 
-// a6: smallest S with about one wave of CTAs (2 resident per SM) and >= 2 KV tiles per split.
+// a6: the attention kernel runs one persistent CTA per SM over work items (attn.cu): per KV group and split,
+// floor(n_qt/2) pair items (both streams walk the split's tiles: ceil(T/S) steps) and n_qt%2 single items (the two
+// streams share the tiles: half the steps); item i goes to CTA i mod num_sms, pair items first.  The model below
+// scores a split count by the busiest CTA's steps (+ a fixed per-item cost) and, when S > 1, the combine kernel's
+// launch and its 2*S*rows*d*4 bytes of partial traffic; the cheapest S wins (ties -> smaller S).
+double split_cost_us(const Dims &d, int S, int sms) {
+    const int T = kv_tiles(d), BG = d.B * d.H_kv;
+    const int n_qt = (d.rows_g + kTileM - 1) / kTileM, n_pairs = n_qt / 2, n_single = n_qt & 1;
+    const double kStepUs = 1.3, kItemSteps = 1.5, kLaunchUs = 3.0, kHbmBytesPerUs = 6.0e6;
+    const int64_t na = (int64_t)BG * n_pairs * S, nb = (int64_t)BG * n_single * S;
+    const double ca = (T + S - 1) / S + kItemSteps, cb = ((T + S - 1) / S + 1) / 2 + kItemSteps;
+    // CTA c receives items c, c + sms, ...: those below na cost ca, the rest cb
+    double worst = 0.0;
+    for (int c = 0; c < sms; ++c) {
+        const int64_t total = (na + nb > c) ? (na + nb - c - 1) / sms + 1 : 0;
+        const int64_t a = (na > c) ? (na - c - 1) / sms + 1 : 0;
+        const double load = a * ca + (total - a) * cb;
+        if (load > worst) worst = load;
+    }
+    double us = worst * kStepUs;
+    if (S > 1) us += kLaunchUs + 2.0 * S * (double)d.B * d.H * d.L * d.d * 4.0 / kHbmBytesPerUs;
+    return us;
+}
+
 int auto_splits(const Dims &d, int num_sms) {
-    const int T = kv_tiles(d), M = m_tiles(d);
-    const int slots = 2 * (num_sms > 0 ? num_sms : 148);
-    int S = 1;
-    while (M * S < slots && T / (S + 1) >= 2) ++S;
-    return S;
+    const int sms = num_sms > 0 ? num_sms : 148;
+    const int T = kv_tiles(d);
+    const int Smax = T < 64 ? T : 64;
+    int best = 1;
+    double best_us = split_cost_us(d, 1, sms);
+    for (int S = 2; S <= Smax; ++S) {
+        const double us = split_cost_us(d, S, sms);
+        if (us < best_us * 0.97) {      // a split must pay for itself by a clear margin
+            best_us = us;
+            best = S;
+        }
+    }
+    return best;
 }
 
 int effective_splits(const Dims &d, int n_splits, int num_sms) {
