@@ -27,13 +27,13 @@ __device__ long long *g_pdllm_trace = nullptr;
 extern "C" int pdllm_debug_set_trace(void *dev_buf) {
     return (int)cudaMemcpyToSymbol(g_pdllm_trace, &dev_buf, sizeof(void *));
 }
-#define PDLLM_TRACE_DECL(role) int tr_n = 0; const int tr_role = (role);
+#define PDLLM_TRACE_DECL(role) \
+    longlong2 *tr_p = (blockIdx.x == 0 && g_pdllm_trace) ? reinterpret_cast<longlong2 *>(g_pdllm_trace) + (role) * 4096 : nullptr; \
+    longlong2 *const tr_end = tr_p + 4096;
 #define PDLLM_TR(code, arg)                                                                       \
     do {                                                                                          \
-        if (blockIdx.x == 0 && g_pdllm_trace && tr_n < 4096) {                                    \
-            g_pdllm_trace[(tr_role * 4096 + tr_n) * 2] = clock64();                               \
-            g_pdllm_trace[(tr_role * 4096 + tr_n) * 2 + 1] = ((long long)(code) << 32) | (unsigned)(arg); \
-            ++tr_n;                                                                               \
+        if (tr_p && tr_p < tr_end) {                                                              \
+            *tr_p++ = make_longlong2(clock64(), ((long long)(code) << 32) | (unsigned)(arg));     \
         }                                                                                         \
     } while (0)
 #else
@@ -52,7 +52,6 @@ constexpr int kMmaWarp0 = 12;
 constexpr int kAttnThreads = 2 * kSoftmaxThreads + kProducerThreads + 32;
 constexpr int kInvalidRow = INT32_MIN;
 constexpr float kRescaleThreshold = 8.0f;                 // log2 units: P stays <= 2^8 between reference-max updates
-constexpr int kMaxPending = 4;                            // cp.async groups in flight per producer thread
 
 struct AttnParams {
     const uint16_t *Q, *Kc, *Vc, *Kd, *Vd;
@@ -92,6 +91,7 @@ __device__ __forceinline__ Item decode_item(const AttnParams &p, int i) {
     return it;
 }
 
+
 template <int D>
 struct AttnCfg {
     static constexpr int kPanels = D / 64;                   // 64-column (128-byte) panels per row
@@ -124,6 +124,59 @@ __device__ __forceinline__ void umma_ts_lohi(uint32_t d_tmem, uint32_t a_tmem, u
         "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], db, %4, p;\n\t}"
         ::"r"(d_tmem), "r"(a_tmem), "r"(b_lo), "r"(desc_hi), "r"(idesc), "r"(accumulate)
         : "memory");
+}
+
+// ---- packed fp32x2 arithmetic (sm_100): two lanes per instruction
+__device__ __forceinline__ uint64_t pack_f32x2(float lo, float hi) {
+    uint64_t r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ uint64_t pack_u32x2(uint32_t lo, uint32_t hi) {
+    uint64_t r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "r"(lo), "r"(hi));
+    return r;
+}
+__device__ __forceinline__ void unpack_f32x2(uint64_t v, float &lo, float &hi) {
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ uint64_t fma_f32x2(uint64_t a, uint64_t b, uint64_t c) {
+    uint64_t d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+__device__ __forceinline__ uint64_t add_f32x2(uint64_t a, uint64_t b) {
+    uint64_t d;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+
+constexpr float kSumLimit = 8192.f;                       // a 32-column chunk's row sum above 2^13 triggers a rescale
+
+// Rare path of the single-pass softmax (kept out of line so the hot loop stays small): multiply this row's O
+// accumulator (o_chunks x 32 columns) and the first p_chunks 16-column packed-bf16 P chunks of the current tile by f,
+// an exact power of two.
+__device__ __noinline__ void rescale_tile(uint32_t tS, uint32_t tO, int p_chunks, int o_chunks, float f) {
+    for (int ch = 0; ch < o_chunks; ++ch) {
+        uint32_t o[32];
+        tmem_ld32(tO + 32u * ch, o);
+        tmem_wait_ld();
+#pragma unroll
+        for (int e = 0; e < 32; ++e) o[e] = __float_as_uint(__uint_as_float(o[e]) * f);
+        tmem_st32(tO + 32u * ch, o);
+    }
+    for (int c0 = 0; c0 < p_chunks; ++c0) {
+        uint32_t pw16[16];
+        tmem_ld16(tS + 16u * c0, pw16);
+        tmem_wait_ld();
+#pragma unroll
+        for (int e = 0; e < 16; ++e) {
+            const float lo = __uint_as_float(pw16[e] << 16) * f, hi = __uint_as_float(pw16[e] & 0xffff0000u) * f;
+            pw16[e] = pack_bf16x2(lo, hi);
+        }
+        tmem_st16(tS + 16u * c0, pw16);
+    }
+    tmem_wait_st();
 }
 
 template <int D>
@@ -183,41 +236,21 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
         // 128B-swizzle term (c ^ row) & 7 is x7 ^ (i*RPI & 7) with x7 = (c & 7) ^ rsub
         const uint32_t dst_thread = dst_pc + (uint32_t)(pw * 32 + rsub) * 128u;
         const uint32_t x7 = (uint32_t)((c & 7) ^ rsub);
-        uint32_t pend0 = 0, pend1 = 0, pend2 = 0, pend3 = 0;   // barriers of the committed, unpublished groups (oldest first)
-        int np = 0;
-        static_assert(kMaxPending == 4, "the pending list is four registers");
-        auto flush_one = [&]() {                          // oldest group has landed -> publish it
-            fence_proxy_async_smem();
-            mbar_arrive(pend0);
-            pend0 = pend1;
-            pend1 = pend2;
-            pend2 = pend3;
-            --np;
+        // Completion is signalled by the hardware: cp.async.mbarrier.arrive.noinc makes the tile's "full" barrier
+        // (count = 128 producer threads) track all cp.async this thread issued so far, so the producers never wait
+        // for their own loads; the MMA warp crosses from the generic to the async proxy with a fence after its wait.
+        auto publish = [&](uint32_t b) {
+            asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(b) : "memory");
         };
-        auto flush_all = [&]() {
-            cp_async_wait<0>();
-            while (np > 0) flush_one();
+        auto wait_free = [&](uint32_t b, uint32_t parity) { mbar_wait(b, parity); };
+        // The cp.async of this thread for one tile: rows pw*32 + i*RPI + rsub (i < 16 at D = 128), chunk c.
+        // destination offset of the i-th row inside a tile
+        auto dst_of = [&](int i) {
+            return dst_thread + (uint32_t)(i * kRowsPerInstr) * 128u + ((x7 ^ (uint32_t)((i * kRowsPerInstr) & 7)) << 4);
         };
-        auto track = [&](uint32_t b) {                    // the group just committed completes barrier b
-            if (np == 0) pend0 = b;
-            else if (np == 1) pend1 = b;
-            else if (np == 2) pend2 = b;
-            else pend3 = b;
-            if (++np == kMaxPending) {
-                cp_async_wait<kMaxPending - 1>();
-                flush_one();
-            }
-        };
-        // a blocking wait on a consumer-driven barrier never holds back landed loads (so it cannot deadlock)
-        auto wait_free = [&](uint32_t b, uint32_t parity) {
-            if (!mbar_try_wait(b, parity)) {
-                flush_all();
-                mbar_wait(b, parity);
-            }
-        };
-        // the cp.async of this thread for one tile: rows pw*32 + i*RPI + rsub, chunk c; the row addresses live one
-        // per lane (lane = row inside the warp's 32) and are fetched by shuffle; address 0 = zero-fill
-        auto issue_rows = [&](uint32_t dst_tile, uint32_t my_lo, uint32_t my_hi, const void *dummy) {
+        // generic: the row addresses live one per lane (lane = row inside the warp's 32), fetched by shuffle; 0 = zero-fill
+        auto issue_rows = [&](uint32_t dst_tile, uint64_t my_addr, const void *dummy) {
+            const uint32_t my_lo = (uint32_t)my_addr, my_hi = (uint32_t)(my_addr >> 32);
 #pragma unroll
             for (int i = 0; i < kChunksPerRow; ++i) {
                 const int rl = i * kRowsPerInstr + rsub;
@@ -225,9 +258,27 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
                 const uint64_t row_addr = ((uint64_t)hi << 32) | lo;
                 const bool ok = row_addr != 0ull;
                 const uint64_t src = ok ? row_addr + (uint64_t)(c * 16) : reinterpret_cast<uint64_t>(dummy);
-                const uint32_t sw = (x7 ^ (uint32_t)((i * kRowsPerInstr) & 7)) << 4;
-                cp_async16_zfill(dst_tile + dst_thread + (uint32_t)(i * kRowsPerInstr) * 128u + sw,
-                                 reinterpret_cast<const void *>(src), ok ? 16u : 0u);
+                cp_async16_zfill(dst_tile + dst_of(i), reinterpret_cast<const void *>(src), ok ? 16u : 0u);
+            }
+        };
+        // prefix-only tile: every row is a cache row; one 32-bit byte offset per row is shuffled and added to the
+        // group's K (and V) base, which already carries this lane's chunk column
+        auto issue_rows_pre = [&](uint32_t dst_k, uint32_t dst_v, uint32_t my_off, uint64_t kbase_c, uint64_t vbase_c,
+                                  bool do_k, bool do_v) {
+#pragma unroll
+            for (int i = 0; i < kChunksPerRow; ++i) {
+                const uint32_t off = __shfl_sync(0xffffffffu, my_off, i * kRowsPerInstr + rsub);
+                if (do_k) cp_async16(dst_k + dst_of(i), reinterpret_cast<const void *>(kbase_c + off));
+                if (do_v) cp_async16(dst_v + dst_of(i), reinterpret_cast<const void *>(vbase_c + off));
+            }
+        };
+        // decode-only tile: consecutive rows of K_dec / V_dec, no indices at all
+        auto issue_rows_dec = [&](uint32_t dst_k, uint32_t dst_v, uint64_t krow0_c, uint64_t vrow0_c, bool do_k, bool do_v) {
+#pragma unroll
+            for (int i = 0; i < kChunksPerRow; ++i) {
+                const uint64_t o = (uint64_t)(i * kRowsPerInstr) * (uint64_t)(D * 2);
+                if (do_k) cp_async16(dst_k + dst_of(i), reinterpret_cast<const void *>(krow0_c + o));
+                if (do_v) cp_async16(dst_v + dst_of(i), reinterpret_cast<const void *>(vrow0_c + o));
             }
         };
         uint32_t lq = 0;                                  // ring load counter (continues across items)
@@ -242,63 +293,108 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
             // the group's K <= 64 chunk ids live in two registers per lane (lane l: ids[l], ids[l + 32])
             const int ids_lo = lane < p.K ? __ldg(p.ids + bg * p.K + lane) : 0;
             const int ids_hi = lane + 32 < p.K ? __ldg(p.ids + bg * p.K + lane + 32) : 0;
-            // a3: virtual row -> cache row (>= 0) / decode row (< 0) / invalid; one row per producer thread
-            auto row_index = [&](int tile) {
+            // a3: virtual row -> cache row (>= 0) / decode row (< 0) / invalid; one row per producer thread.  The index
+            // is kept as (base, raw) with raw = the keep-list entry still in flight: the sum is only formed when the
+            // row is issued, one load later, so the global load latency hides behind the previous tile's cp.async.
+            int nx_base = 0, nx_raw = 0;
+            auto prefetch_index = [&](int tile) {
                 const int vr = tile * kTileN + pt;
                 const bool pre = vr < p.S_pre;
                 const int k = pre ? vr / p.Bk : 0, t = vr - k * p.Bk;
                 const int n_lo = __shfl_sync(0xffffffffu, ids_lo, k & 31), n_hi = __shfl_sync(0xffffffffu, ids_hi, k & 31);
                 const int n = k < 32 ? n_lo : n_hi;
-                int idx = kInvalidRow;
-                if (pre) idx = n * p.Cp + (keep ? __ldg(keep + (int64_t)n * p.Bk + t) : t);
-                else if (vr < p.S_kv) idx = -(vr - p.S_pre) - 1;
-                return idx;
+                nx_raw = 0;
+                if (pre && keep) nx_raw = __ldg(keep + (int64_t)n * p.Bk + t);
+                nx_base = pre ? n * p.Cp + (keep ? 0 : t) : (vr < p.S_kv ? -(vr - p.S_pre) - 1 : kInvalidRow);
             };
-            int idx_next = row_index(it.t0);
-            for (int jt = 0; jt < it.nt; ++jt, lq += 2) {
-                const int my_idx = idx_next;
-                if (pt == 0) PDLLM_TR(10, lq);
-                if (jt + 1 < it.nt) idx_next = row_index(it.t0 + jt + 1);   // in flight while this tile is issued
-                const int slot_k = (int)(lq % ST), slot_v = (int)((lq + 1) % ST);
-                if (lq >= (uint32_t)ST) wait_free(kv_free(slot_k), ((lq / ST) - 1) & 1u);
-                if (lq + 1 >= (uint32_t)ST) wait_free(kv_free(slot_v), (((lq + 1) / ST) - 1) & 1u);
-                if (pt == 0) PDLLM_TR(11, lq);
-                // this thread's row (pw*32 + lane) as global byte addresses in K and V; 0 = beyond the sequence
-                const bool in_cache = my_idx >= 0;
-                const int64_t row_off = in_cache ? (int64_t)my_idx * D : (int64_t)(-my_idx - 1) * D;
-                const bool valid = my_idx != kInvalidRow;
-                const uint64_t ka = valid ? reinterpret_cast<uint64_t>((in_cache ? Kc : Kd) + row_off) : 0ull;
-                const uint64_t va = valid ? reinterpret_cast<uint64_t>((in_cache ? Vc : Vd) + row_off) : 0ull;
-                issue_rows(sKV(slot_k), (uint32_t)ka, (uint32_t)(ka >> 32), Kc);
-                cp_async_commit();
-                track(kv_full(slot_k));
-                issue_rows(sKV(slot_v), (uint32_t)va, (uint32_t)(va >> 32), Vc);
-                cp_async_commit();
-                if (pt == 0) PDLLM_TR(12, lq);
-                track(kv_full(slot_v));
-                if (pt == 0) PDLLM_TR(13, np);
-                if (jt == 0) {
-                    // the item's Q tile(s), once the previous item's Q*K^T are all done
-                    if (n_done > 0) wait_free(bar(BAR_QFREE), (uint32_t)(n_done - 1) & 1u);
-                    const uint16_t *Qg = p.Q + bg * p.rows_g * D;
-                    const int n_q = it.modeA ? 2 : 1;
-                    for (int s = 0; s < n_q; ++s) {
+            // the item's Q tile(s), once the previous item's Q*K^T are all done
+            auto load_q = [&]() {
+                if (n_done > 0) wait_free(bar(BAR_QFREE), (uint32_t)(n_done - 1) & 1u);
+                const uint16_t *Qg = p.Q + bg * p.rows_g * D;
+                const int n_q = it.modeA ? 2 : 1;
+                for (int s = 0; s < n_q; ++s) {
 #pragma unroll
-                        for (int i = 0; i < kChunksPerRow; ++i) {
-                            const int r = pw * 32 + i * kRowsPerInstr + rsub;
-                            const int qr = (it.q0 + s) * kTileM + r;
-                            const bool ok = qr < p.rows_g;
-                            const uint32_t sw = (x7 ^ (uint32_t)((i * kRowsPerInstr) & 7)) << 4;
-                            cp_async16_zfill(sQ(s) + dst_thread + (uint32_t)(i * kRowsPerInstr) * 128u + sw,
-                                             ok ? Qg + (int64_t)qr * D + c * 8 : Qg, ok ? 16u : 0u);
-                        }
+                    for (int i = 0; i < kChunksPerRow; ++i) {
+                        const int r = pw * 32 + i * kRowsPerInstr + rsub;
+                        const int qr = (it.q0 + s) * kTileM + r;
+                        const bool ok = qr < p.rows_g;
+                        const uint32_t sw = (x7 ^ (uint32_t)((i * kRowsPerInstr) & 7)) << 4;
+                        cp_async16_zfill(sQ(s) + dst_thread + (uint32_t)(i * kRowsPerInstr) * 128u + sw,
+                                         ok ? Qg + (int64_t)qr * D + c * 8 : Qg, ok ? 16u : 0u);
                     }
-                    cp_async_commit();
-                    track(bar(BAR_QFULL));
                 }
+                publish(bar(BAR_QFULL));
+            };
+            // this thread's row (pw*32 + lane) of a tile as a global byte address in K or V; 0 = beyond the sequence
+            auto row_addr = [&](int idx, bool is_v) -> uint64_t {
+                if (idx == kInvalidRow) return 0ull;
+                const bool in_cache = idx >= 0;
+                const int64_t row_off = in_cache ? (int64_t)idx * D : (int64_t)(-idx - 1) * D;
+                const uint16_t *base = in_cache ? (is_v ? Vc : Kc) : (is_v ? Vd : Kd);
+                return reinterpret_cast<uint64_t>(base + row_off);
+            };
+            auto wait_slot = [&](uint32_t q) {
+                if (q >= (uint32_t)ST) wait_free(kv_free((int)(q % ST)), ((q / ST) - 1) & 1u);
+            };
+            // K and/or V rows of one tile into the given slots
+            const uint64_t kbase_c = reinterpret_cast<uint64_t>(Kc + c * 8), vbase_c = reinterpret_cast<uint64_t>(Vc + c * 8);
+            auto load_tile = [&](int tile, int my_idx, uint32_t dst_k, uint32_t dst_v, bool do_k, bool do_v) {
+                const int r0 = tile * kTileN;
+                if (r0 + kTileN <= p.S_pre) {
+                    issue_rows_pre(dst_k, dst_v, (uint32_t)my_idx * (uint32_t)(D * 2), kbase_c, vbase_c, do_k, do_v);
+                } else if (r0 >= p.S_pre && r0 + kTileN <= p.S_kv) {
+                    const int64_t e0 = ((int64_t)(r0 - p.S_pre + pw * 32 + rsub)) * D + c * 8;
+                    issue_rows_dec(dst_k, dst_v, reinterpret_cast<uint64_t>(Kd + e0), reinterpret_cast<uint64_t>(Vd + e0), do_k, do_v);
+                } else {
+                    if (do_k) issue_rows(dst_k, row_addr(my_idx, false), Kc);
+                    if (do_v) issue_rows(dst_v, row_addr(my_idx, true), Vc);
+                }
+            };
+            if (it.modeA) {
+                // tile by tile, K and V together (one index computation, one cp.async group): loads 2*jt and 2*jt + 1
+                prefetch_index(it.t0);
+                for (int jt = 0; jt < it.nt; ++jt, lq += 2) {
+                    const int my_idx = nx_base + nx_raw;
+                    if (pt == 0) PDLLM_TR(10, lq);
+                    if (jt + 1 < it.nt) prefetch_index(it.t0 + jt + 1);         // in flight while this tile is issued
+                    wait_slot(lq);
+                    wait_slot(lq + 1);
+                    if (pt == 0) PDLLM_TR(11, lq);
+                    load_tile(it.t0 + jt, my_idx, sKV((int)(lq % ST)), sKV((int)((lq + 1) % ST)), true, true);
+                    if (pt == 0) PDLLM_TR(12, lq);
+                    publish(kv_full((int)(lq % ST)));
+                    publish(kv_full((int)((lq + 1) % ST)));
+                    if (jt == 0) load_q();
+                }
+            } else {
+                // one tile per load, in the MMA warp's consumption order K(t0); { K(t0+i+1), V(t0+i) }; V(t0+nt-1)
+                // (each tile has a single user); a tile's indices are computed once and serve its K and its V load
+                auto load_one = [&](int tile, int idx, bool is_v) {
+                    if (pt == 0) PDLLM_TR(10, lq);
+                    wait_slot(lq);
+                    if (pt == 0) PDLLM_TR(11, lq);
+                    const uint32_t dst = sKV((int)(lq % ST));
+                    load_tile(tile, idx, dst, dst, !is_v, is_v);
+                    if (pt == 0) PDLLM_TR(12, lq);
+                    publish(kv_full((int)(lq % ST)));
+                    ++lq;
+                };
+                prefetch_index(it.t0);
+                int idx_cur = nx_base + nx_raw;
+                if (it.nt > 1) prefetch_index(it.t0 + 1);
+                load_one(it.t0, idx_cur, false);
+                if (it.nt == 1) load_q();
+                for (int i = 0; i + 1 < it.nt; ++i) {
+                    const int idx_new = nx_base + nx_raw;                       // tile t0 + i + 1
+                    if (i + 2 < it.nt) prefetch_index(it.t0 + i + 2);
+                    load_one(it.t0 + i + 1, idx_new, false);
+                    if (i == 0) load_q();                                       // Q goes in after the first two K tiles
+                    load_one(it.t0 + i, idx_cur, true);
+                    idx_cur = idx_new;
+                }
+                load_one(it.t0 + it.nt - 1, idx_cur, true);
             }
         }
-        flush_all();
     } else if (warp == kMmaWarp0) {
         // =============================== MMA issuer ===============================
         // One warp issues both streams' MMAs in the fixed order QK(0,0) QK(1,0) { PV(0,j) QK(0,j+1) PV(1,j) QK(1,j+1) }:
@@ -319,15 +415,19 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
             const int n_s[2] = {it.modeA ? it.nt : (it.nt + 1) / 2, it.modeA ? it.nt : it.nt / 2};
             const int qk_total = n_s[0] + n_s[1];
             int qk_issued = 0;
+            uint32_t lq = lq_base;                        // mode B: loads are consumed strictly in ring order
             auto tile_of = [&](int s, int j) { return it.modeA ? it.t0 + j : it.t0 + 2 * j + s; };
             auto n_mma_of = [&](int tile) { return (uint32_t)((min(kTileN, p.S_kv - tile * kTileN) + 15) & ~15); };
             auto issue_qk = [&](int s, int j) {
                 const int tile = tile_of(s, j);
-                const uint32_t q = lq_base + 2u * (uint32_t)(tile - it.t0);
+                const uint32_t q = it.modeA ? lq_base + 2u * (uint32_t)(tile - it.t0) : lq++;
                 const int slot = (int)(q % ST);
                 const bool release = !it.modeA || s == 1;     // last user of this K tile
                 if (lane == 0) PDLLM_TR(20, s);
-                if (!it.modeA || s == 0) mbar_wait(kv_full(slot), (q / ST) & 1u);
+                if (!it.modeA || s == 0) {
+                    mbar_wait(kv_full(slot), (q / ST) & 1u);
+                    fence_proxy_async_smem();             // cp.async (generic proxy) wrote the tile
+                }
                 tc_fence_after();
                 const bool last_qk = ++qk_issued == qk_total;
                 if (elect_one()) {
@@ -355,14 +455,17 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
                 for (int s = 0; s < 2; ++s) {
                     if (j >= n_s[s]) continue;
                     const int tile = tile_of(s, j);
-                    const uint32_t q = lq_base + 2u * (uint32_t)(tile - it.t0) + 1u;
+                    const uint32_t q = it.modeA ? lq_base + 2u * (uint32_t)(tile - it.t0) + 1u : lq++;
                     const int slot = (int)(q % ST);
                     const bool release = !it.modeA || s == 1;     // last user of this V tile
                     if (lane == 0) PDLLM_TR(23, s);
                     mbar_wait(bar(BAR_PREADY0 + s), n_pready[s]++ & 1u);
                     if (lane == 0) PDLLM_TR(24, s);
                     if (j == 0 && n_oready[s] > 0) mbar_wait(bar(BAR_OFREE0 + s), (n_oready[s] - 1) & 1u);
-                    if (!it.modeA || s == 0) mbar_wait(kv_full(slot), (q / ST) & 1u);
+                    if (!it.modeA || s == 0) {
+                        mbar_wait(kv_full(slot), (q / ST) & 1u);
+                        fence_proxy_async_smem();
+                    }
                     tc_fence_after();
                     if (lane == 0) PDLLM_TR(25, s);
                     const int ksteps = (int)(n_mma_of(tile) >> 4);
@@ -415,19 +518,26 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
                     tmem_st32(tO + 32u * ch, o);
                 }
             };
-            // one 32-column chunk of a FULL tile: P = 2^(c2*S - m_ref) as packed bf16, row sum, raw max
-            auto chunk_exp = [&](const uint32_t(&v)[32], uint32_t(&w)[16], float &csum, float &cmax) {
-                float ls[4] = {0.f, 0.f, 0.f, 0.f}, mx[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
+            // one 32-column chunk of a FULL tile: P = 2^(c2*S - m_ref) as packed bf16 and its row sum; packed f32x2
+            // arithmetic (one FFMA2 / FADD2 per two columns), the exponentials on the MUFU pipe
+            auto chunk_exp = [&](const uint32_t(&v)[32], uint32_t(&w)[16]) {
+                const uint64_t c2v = pack_f32x2(p.c2, p.c2), mv = pack_f32x2(-m_ref, -m_ref);
+                uint64_t acc0 = 0ull, acc1 = 0ull;
 #pragma unroll
-                for (int e = 0; e < 32; e += 2) {
-                    const float x0 = __uint_as_float(v[e]), x1 = __uint_as_float(v[e + 1]);
-                    const float p0 = ex2_approx(fmaf(x0, p.c2, -m_ref)), p1 = ex2_approx(fmaf(x1, p.c2, -m_ref));
-                    mx[(e >> 1) & 3] = fmaxf(mx[(e >> 1) & 3], fmaxf(x0, x1));
-                    ls[(e >> 1) & 3] += p0 + p1;
+                for (int e = 0; e < 32; e += 4) {
+                    float x0, x1, x2, x3;
+                    unpack_f32x2(fma_f32x2(pack_u32x2(v[e], v[e + 1]), c2v, mv), x0, x1);
+                    unpack_f32x2(fma_f32x2(pack_u32x2(v[e + 2], v[e + 3]), c2v, mv), x2, x3);
+                    const float p0 = ex2_approx(x0), p1 = ex2_approx(x1), p2 = ex2_approx(x2), p3 = ex2_approx(x3);
+                    acc0 = add_f32x2(acc0, pack_f32x2(p0, p1));
+                    acc1 = add_f32x2(acc1, pack_f32x2(p2, p3));
                     w[e >> 1] = pack_bf16x2(p0, p1);
+                    w[(e >> 1) + 1] = pack_bf16x2(p2, p3);
                 }
-                csum = (ls[0] + ls[1]) + (ls[2] + ls[3]);
-                cmax = fmaxf(fmaxf(mx[0], mx[1]), fmaxf(mx[2], mx[3]));
+                float s0, s1, s2, s3;
+                unpack_f32x2(acc0, s0, s1);
+                unpack_f32x2(acc1, s2, s3);
+                return (s0 + s1) + (s2 + s3);
             };
             for (int j = 0; j < n_mine; ++j) {
                 const int tile = it.modeA ? it.t0 + j : it.t0 + 2 * j + s;
@@ -436,53 +546,58 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
                 mbar_wait(bar(BAR_SREADY0 + s), n_sready++ & 1u);
                 tc_fence_after();
                 if (row == 0) PDLLM_TR(31, j);
-                if (n_valid == kTileN && j > 0) {
-                    // Single pass with the current reference max, TMEM loads one chunk ahead of the arithmetic.  A
-                    // chunk whose max outgrew the reference (rare) raises it by a whole number of octaves BEFORE its P is
+                if (n_valid == kTileN) {
+                    if (j == 0) {
+                        // first tile of the stream: its row max becomes the reference (one extra pass over S)
+                        uint32_t v0[32], v1[32];
+                        float mx[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
+#pragma unroll 1
+                        for (int h = 0; h < 2; ++h) {
+                            tmem_ld32(tS + 64u * h, v0);
+                            tmem_ld32(tS + 64u * h + 32u, v1);
+                            tmem_wait_ld();
+#pragma unroll
+                            for (int e = 0; e < 32; ++e) mx[e & 3] = fmaxf(mx[e & 3], fmaxf(__uint_as_float(v0[e]), __uint_as_float(v1[e])));
+                        }
+                        m_ref = fmaxf(fmaxf(mx[0], mx[1]), fmaxf(mx[2], mx[3])) * p.c2;
+                    }
+                    // Single pass with the current reference max, TMEM loads one chunk ahead of the arithmetic.  The
+                    // chunk's row sum doubles as the overflow detector: some P > 2^13 implies sum > 2^13 (kSumLimit).
+                    // A chunk that trips it (rare) raises the reference by a whole number of octaves BEFORE its P is
                     // stored: l, O and the P chunks already stored are rescaled by an exact power of two.
                     float lsum = 0.f;
                     uint32_t va[32], vb[32];
                     auto do_chunk = [&](const uint32_t(&v)[32], int ch) {
                         uint32_t w[16];
-                        float csum, cmax;
-                        chunk_exp(v, w, csum, cmax);
-                        const float over = cmax * p.c2 - m_ref;
-                        if (__any_sync(0xffffffffu, over > kRescaleThreshold)) {
-                            const float up = over > kRescaleThreshold ? ceilf(over) : 0.f;
+                        float csum = chunk_exp(v, w);
+                        while (__any_sync(0xffffffffu, !(csum <= kSumLimit))) {
+                            float cmax = -INFINITY;
+#pragma unroll
+                            for (int e = 0; e < 32; ++e) cmax = fmaxf(cmax, __uint_as_float(v[e]));
+                            const float over = cmax * p.c2 - m_ref;
+                            const float up = !(csum <= kSumLimit) ? fmaxf(ceilf(over), 1.f) : 0.f;
                             const float f = ex2_approx(-up);      // exact power of two (1 for rows that are fine)
                             l *= f;
                             lsum *= f;
                             tmem_wait_st();
-                            scale_O(f);
-                            for (int c0 = 0; c0 < ch; ++c0) {     // P chunks of this tile stored so far
-                                uint32_t pw16[16];
-                                tmem_ld16(tS + 16u * c0, pw16);
-                                tmem_wait_ld();
-#pragma unroll
-                                for (int e = 0; e < 16; ++e) {
-                                    const float lo = __uint_as_float(pw16[e] << 16) * f, hi = __uint_as_float(pw16[e] & 0xffff0000u) * f;
-                                    pw16[e] = pack_bf16x2(lo, hi);
-                                }
-                                tmem_st16(tS + 16u * c0, pw16);
-                            }
+                            rescale_tile(tS, tO, ch, D / 32, f);
                             m_ref += up;
-                            chunk_exp(v, w, csum, cmax);
+                            csum = chunk_exp(v, w);
                         }
                         lsum += csum;
                         tmem_st16(tS + 16u * ch, w);
                     };
                     tmem_ld32(tS, va);
                     tmem_wait_ld();
-                    tmem_ld32(tS + 32u, vb);
-                    do_chunk(va, 0);
-                    tmem_wait_ld();
-                    tmem_ld32(tS + 64u, va);
-                    do_chunk(vb, 1);
-                    tmem_wait_ld();
-                    tmem_ld32(tS + 96u, vb);
-                    do_chunk(va, 2);
-                    tmem_wait_ld();
-                    do_chunk(vb, 3);
+#pragma unroll 1
+                    for (int h = 0; h < 2; ++h) {
+                        tmem_ld32(tS + 64u * h + 32u, vb);
+                        do_chunk(va, 2 * h);
+                        tmem_wait_ld();
+                        if (h == 0) tmem_ld32(tS + 64u, va);
+                        do_chunk(vb, 2 * h + 1);
+                        if (h == 0) tmem_wait_ld();
+                    }
                     l += lsum;
                 } else {
                     // first tile of the stream or a ragged tail tile: max pass, then exp pass with column masks

@@ -35,6 +35,8 @@ int resolve(const pdllm_shape *sh, bool has_keep, Dims *out) {
     const int64_t cache_rows = (int64_t)sh->B * sh->H_kv * sh->N * (sh->C + 1);
     if (cache_rows >= (1ll << 31)) return PDLLM_ERR_SHAPE;
     if ((int64_t)sh->K * sh->Bk + sh->L_s >= (1ll << 30)) return PDLLM_ERR_SHAPE;
+    // one KV group's cache is addressed with 32-bit byte offsets by the gather (attn.cu)
+    if ((int64_t)sh->N * (sh->C + 1) * sh->d * 2 >= (1ll << 32)) return PDLLM_ERR_SHAPE;
     if ((int64_t)sh->B * sh->H_kv > 65535) return PDLLM_ERR_SHAPE;
     Dims d;
     d.B = sh->B; d.H = sh->H; d.H_kv = sh->H_kv; d.G = sh->H / sh->H_kv; d.d = sh->d;
