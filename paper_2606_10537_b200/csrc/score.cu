@@ -149,52 +149,109 @@ score_kernel(const ScoreParams p, const __grid_constant__ CUtensorMap tmap128, c
         __syncwarp();
     } else {
         // =============================== softmax (thread = row) ===============================
+        // Per chunk a running (reference max m_ref, sum l) in log2 units.  The chunk's first tile fixes m_ref with a max
+        // pass; later tiles take one exp pass against it.  A 32-column block whose row sum exceeds kSumLimit (some
+        // logit outgrew the reference by > 13 octaves; rare) raises m_ref by whole octaves and is recomputed.
         const uint32_t lane_base = (uint32_t)(warp * 32) << 16;
         const bool row_ok = mt * kTileM + tid < p.rows;
+        constexpr float kSumLimit = 8192.f;
         int q = 0;
         for (int n = n0; n < n1; ++n) {
-            float m_run = -INFINITY, l = 0.f;
+            float m_ref = -INFINITY, l = 0.f;
+            // sum over 32 columns of 2^(c2*x - m_ref): packed f32x2 arithmetic, exponentials on the MUFU pipe
+            auto block_sum = [&](const uint32_t(&v)[32]) {
+                const uint64_t c2v = pack_f32x2(p.c2, p.c2), mv = pack_f32x2(-m_ref, -m_ref);
+                uint64_t acc0 = 0ull, acc1 = 0ull;
+#pragma unroll
+                for (int e = 0; e < 32; e += 4) {
+                    float x0, x1, x2, x3;
+                    unpack_f32x2(fma_f32x2(pack_u32x2(v[e], v[e + 1]), c2v, mv), x0, x1);
+                    unpack_f32x2(fma_f32x2(pack_u32x2(v[e + 2], v[e + 3]), c2v, mv), x2, x3);
+                    acc0 = add_f32x2(acc0, pack_f32x2(ex2_approx(x0), ex2_approx(x1)));
+                    acc1 = add_f32x2(acc1, pack_f32x2(ex2_approx(x2), ex2_approx(x3)));
+                }
+                float s0, s1, s2, s3;
+                unpack_f32x2(acc0, s0, s1);
+                unpack_f32x2(acc1, s2, s3);
+                return (s0 + s1) + (s2 + s3);
+            };
+            auto add_block = [&](const uint32_t(&v)[32]) {
+                float bs = block_sum(v);
+                while (__any_sync(0xffffffffu, !(bs <= kSumLimit))) {
+                    float bmax = -INFINITY;
+#pragma unroll
+                    for (int e = 0; e < 32; ++e) bmax = fmaxf(bmax, __uint_as_float(v[e]));
+                    const float up = !(bs <= kSumLimit) ? fmaxf(ceilf(bmax * p.c2 - m_ref), 1.f) : 0.f;
+                    l *= ex2_approx(-up);
+                    m_ref += up;
+                    bs = block_sum(v);
+                }
+                l += bs;
+            };
             for (int tt = 0; tt < tiles_per_chunk; ++tt, ++q) {
                 const int buf = q & 1;
                 const int valid = min(kTileN, p.Cp - tt * kTileN);
-                const int nchunks = (((valid + 15) & ~15) + 31) >> 5;
                 const uint32_t tS = tmem + 128u * buf + lane_base;
                 mbar_wait(s_ready(buf), (q >> 1) & 1);
                 tc_fence_after();
-                for (int ch = 0; ch < nchunks; ++ch) {
-                    uint32_t v[32];
-                    tmem_ld32(tS + 32u * ch, v);
-                    tmem_wait_ld();
-                    if (ch == nchunks - 1) {          // accumulator buffer is free once it is in registers
-                        tc_fence_before();
-                        mbar_arrive(s_free(buf));
-                    }
-                    const int nv = valid - ch * 32;   // valid columns in this 32-column chunk (may exceed 32)
-                    float cmax = -INFINITY;
-                    if (nv >= 32) {
+                if (valid == kTileN) {
+                    uint32_t va[32], vb[32];
+                    if (tt == 0) {
+                        float mx[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
+#pragma unroll 1
+                        for (int h = 0; h < 2; ++h) {
+                            tmem_ld32(tS + 64u * h, va);
+                            tmem_ld32(tS + 64u * h + 32u, vb);
+                            tmem_wait_ld();
 #pragma unroll
-                        for (int e = 0; e < 32; ++e) cmax = fmaxf(cmax, __uint_as_float(v[e]));
-                    } else {
+                            for (int e = 0; e < 32; ++e)
+                                mx[e & 3] = fmaxf(mx[e & 3], fmaxf(__uint_as_float(va[e]), __uint_as_float(vb[e])));
+                        }
+                        m_ref = fmaxf(fmaxf(mx[0], mx[1]), fmaxf(mx[2], mx[3])) * p.c2;
+                    }
+                    // TMEM loads one block ahead of the arithmetic; the accumulator is free once its last block is in registers
+                    tmem_ld32(tS, va);
+                    tmem_wait_ld();
+                    tmem_ld32(tS + 32u, vb);
+                    add_block(va);
+                    tmem_wait_ld();
+                    tmem_ld32(tS + 64u, va);
+                    add_block(vb);
+                    tmem_wait_ld();
+                    tmem_ld32(tS + 96u, vb);
+                    add_block(va);
+                    tmem_wait_ld();
+                    tc_fence_before();
+                    mbar_arrive(s_free(buf));
+                    add_block(vb);
+                } else {
+                    // ragged tail tile of the chunk: online update per 32-column block with column masks
+                    const int nchunks = (((valid + 15) & ~15) + 31) >> 5;
+                    for (int ch = 0; ch < nchunks; ++ch) {
+                        uint32_t v[32];
+                        tmem_ld32(tS + 32u * ch, v);
+                        tmem_wait_ld();
+                        if (ch == nchunks - 1) {
+                            tc_fence_before();
+                            mbar_arrive(s_free(buf));
+                        }
+                        const int nv = valid - ch * 32;
+                        float cmax = -INFINITY;
 #pragma unroll
                         for (int e = 0; e < 32; ++e)
                             if (e < nv) cmax = fmaxf(cmax, __uint_as_float(v[e]));
-                    }
-                    const float m_new = fmaxf(m_run, cmax * p.c2);
-                    float sum = 0.f;
-                    if (nv >= 32) {
-#pragma unroll
-                        for (int e = 0; e < 32; ++e) sum += ex2_approx(fmaf(__uint_as_float(v[e]), p.c2, -m_new));
-                    } else {
+                        const float m_new = fmaxf(m_ref, cmax * p.c2);
+                        float sum = 0.f;
 #pragma unroll
                         for (int e = 0; e < 32; ++e)
                             if (e < nv) sum += ex2_approx(fmaf(__uint_as_float(v[e]), p.c2, -m_new));
+                        l = l * ex2_approx(m_ref - m_new) + sum;
+                        m_ref = m_new;
                     }
-                    l = l * ex2_approx(m_run - m_new) + sum;
-                    m_run = m_new;
                 }
             }
             // chunk n finished: log-mass of this row, summed over the tile's rows (fixed order)
-            float ell = row_ok ? (m_run + lg2_approx(l)) * 0.6931471805599453f : 0.f;
+            float ell = row_ok ? (m_ref + lg2_approx(l)) * 0.6931471805599453f : 0.f;
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) ell += __shfl_xor_sync(0xffffffffu, ell, o);
             if (lane == 0) s_acc[(n - n0) * 4 + warp] = ell;
