@@ -255,6 +255,29 @@ __device__ __forceinline__ uint64_t add_f32x2(uint64_t a, uint64_t b) {
     return d;
 }
 
+// 2^x for two values on the FMA pipe (no MUFU): round-to-nearest split x = n + f, f in [-0.5, 0.5], a degree-4
+// minimax polynomial for 2^f (max relative error 2.7e-6) and n added into the exponent field.  x is clamped to
+// [-126, 127] so that the exponent arithmetic cannot wrap (underflow -> ~1e-38, overflow -> ~1.7e38, never garbage).
+__device__ __forceinline__ void ex2_poly_x2(float x0, float x1, float &r0, float &r1) {
+    x0 = fminf(fmaxf(x0, -126.f), 127.f);
+    x1 = fminf(fmaxf(x1, -126.f), 127.f);
+    const uint64_t x = pack_f32x2(x0, x1);
+    const uint64_t magic = pack_f32x2(12582912.f, 12582912.f), nmagic = pack_f32x2(-12582912.f, -12582912.f);
+    const uint64_t t = add_f32x2(x, magic);                                  // n in the low mantissa bits
+    const uint64_t fl = add_f32x2(t, nmagic);                                // n as a float
+    const uint64_t f = fma_f32x2(fl, pack_f32x2(-1.f, -1.f), x);             // x - n
+    uint64_t p = pack_f32x2(9.570101276e-03f, 9.570101276e-03f);
+    p = fma_f32x2(p, f, pack_f32x2(5.591785908e-02f, 5.591785908e-02f));
+    p = fma_f32x2(p, f, pack_f32x2(2.402474433e-01f, 2.402474433e-01f));
+    p = fma_f32x2(p, f, pack_f32x2(6.931217909e-01f, 6.931217909e-01f));
+    p = fma_f32x2(p, f, pack_f32x2(9.999992847e-01f, 9.999992847e-01f));
+    float p0, p1, t0, t1;
+    unpack_f32x2(p, p0, p1);
+    unpack_f32x2(t, t0, t1);
+    r0 = __int_as_float(__float_as_int(p0) + (__float_as_int(t0) << 23));
+    r1 = __int_as_float(__float_as_int(p1) + (__float_as_int(t1) << 23));
+}
+
 __device__ __forceinline__ uint32_t elect_one() {
     uint32_t pred;
     asm volatile(

@@ -19,6 +19,7 @@ namespace {
 
 constexpr int kScoreThreads = 192;        // 4 softmax warps + TMA warp + MMA warp
 constexpr int kMaxChunksPerCta = 64;
+constexpr bool kPolyShare = true;          // MUFU is co-critical with HBM here (538 M ex2 per C4 launch): offload 1/4
 
 struct ScoreParams {
     const uint16_t *Q;
@@ -161,32 +162,25 @@ score_kernel(const ScoreParams p, const __grid_constant__ CUtensorMap tmap128, c
             // sum over 32 columns of 2^(c2*x - m_ref): packed f32x2 arithmetic, exponentials on the MUFU pipe
             auto block_sum = [&](const uint32_t(&v)[32]) {
                 const uint64_t c2v = pack_f32x2(p.c2, p.c2), mv = pack_f32x2(-m_ref, -m_ref);
-                uint64_t acc0 = 0ull, acc1 = 0ull;
+                float s0 = 0.f, s1 = 0.f, s2 = 0.f, s3 = 0.f;
 #pragma unroll
                 for (int e = 0; e < 32; e += 4) {
                     float x0, x1, x2, x3;
                     unpack_f32x2(fma_f32x2(pack_u32x2(v[e], v[e + 1]), c2v, mv), x0, x1);
                     unpack_f32x2(fma_f32x2(pack_u32x2(v[e + 2], v[e + 3]), c2v, mv), x2, x3);
-                    acc0 = add_f32x2(acc0, pack_f32x2(ex2_approx(x0), ex2_approx(x1)));
-                    acc1 = add_f32x2(acc1, pack_f32x2(ex2_approx(x2), ex2_approx(x3)));
+                    if ((e & 4) == 0 && kPolyShare) {     // a quarter of the exponentials run on the FMA pipe
+                        float r0, r1;
+                        ex2_poly_x2(x0, x1, r0, r1);
+                        s0 += r0;
+                        s1 += r1;
+                    } else {
+                        s0 += ex2_approx(x0);
+                        s1 += ex2_approx(x1);
+                    }
+                    s2 += ex2_approx(x2);
+                    s3 += ex2_approx(x3);
                 }
-                float s0, s1, s2, s3;
-                unpack_f32x2(acc0, s0, s1);
-                unpack_f32x2(acc1, s2, s3);
                 return (s0 + s1) + (s2 + s3);
-            };
-            auto add_block = [&](const uint32_t(&v)[32]) {
-                float bs = block_sum(v);
-                while (__any_sync(0xffffffffu, !(bs <= kSumLimit))) {
-                    float bmax = -INFINITY;
-#pragma unroll
-                    for (int e = 0; e < 32; ++e) bmax = fmaxf(bmax, __uint_as_float(v[e]));
-                    const float up = !(bs <= kSumLimit) ? fmaxf(ceilf(bmax * p.c2 - m_ref), 1.f) : 0.f;
-                    l *= ex2_approx(-up);
-                    m_ref += up;
-                    bs = block_sum(v);
-                }
-                l += bs;
             };
             for (int tt = 0; tt < tiles_per_chunk; ++tt, ++q) {
                 const int buf = q & 1;
@@ -196,34 +190,49 @@ score_kernel(const ScoreParams p, const __grid_constant__ CUtensorMap tmap128, c
                 tc_fence_after();
                 if (valid == kTileN) {
                     uint32_t va[32], vb[32];
-                    if (tt == 0) {
-                        float mx[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
+                    bool max_pass = tt == 0;
+                    float tsum;
+                    for (;;) {
+                        if (max_pass) {
+                            float mx[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
 #pragma unroll 1
-                        for (int h = 0; h < 2; ++h) {
-                            tmem_ld32(tS + 64u * h, va);
-                            tmem_ld32(tS + 64u * h + 32u, vb);
-                            tmem_wait_ld();
+                            for (int h = 0; h < 2; ++h) {
+                                tmem_ld32(tS + 64u * h, va);
+                                tmem_ld32(tS + 64u * h + 32u, vb);
+                                tmem_wait_ld();
 #pragma unroll
-                            for (int e = 0; e < 32; ++e)
-                                mx[e & 3] = fmaxf(mx[e & 3], fmaxf(__uint_as_float(va[e]), __uint_as_float(vb[e])));
+                                for (int e = 0; e < 32; ++e)
+                                    mx[e & 3] = fmaxf(mx[e & 3], fmaxf(__uint_as_float(va[e]), __uint_as_float(vb[e])));
+                            }
+                            const float tm2 = fmaxf(fmaxf(mx[0], mx[1]), fmaxf(mx[2], mx[3])) * p.c2;
+                            if (tt == 0) {
+                                m_ref = tm2;
+                            } else {                      // raise the reference by whole octaves (exact rescale of l)
+                                const float up = fmaxf(ceilf(tm2 - m_ref), 0.f);
+                                l *= ex2_approx(-up);
+                                m_ref += up;
+                            }
                         }
-                        m_ref = fmaxf(fmaxf(mx[0], mx[1]), fmaxf(mx[2], mx[3])) * p.c2;
+                        // TMEM loads one block ahead of the arithmetic
+                        tmem_ld32(tS, va);
+                        tmem_wait_ld();
+                        tmem_ld32(tS + 32u, vb);
+                        tsum = block_sum(va);
+                        tmem_wait_ld();
+                        tmem_ld32(tS + 64u, va);
+                        tsum += block_sum(vb);
+                        tmem_wait_ld();
+                        tmem_ld32(tS + 96u, vb);
+                        tsum += block_sum(va);
+                        tmem_wait_ld();
+                        tsum += block_sum(vb);
+                        // some logit outgrew the reference by > 13 octaves (rare): redo the tile behind a max pass
+                        if (!__any_sync(0xffffffffu, !(tsum <= 4.f * kSumLimit))) break;
+                        max_pass = true;
                     }
-                    // TMEM loads one block ahead of the arithmetic; the accumulator is free once its last block is in registers
-                    tmem_ld32(tS, va);
-                    tmem_wait_ld();
-                    tmem_ld32(tS + 32u, vb);
-                    add_block(va);
-                    tmem_wait_ld();
-                    tmem_ld32(tS + 64u, va);
-                    add_block(vb);
-                    tmem_wait_ld();
-                    tmem_ld32(tS + 96u, vb);
-                    add_block(va);
-                    tmem_wait_ld();
                     tc_fence_before();
                     mbar_arrive(s_free(buf));
-                    add_block(vb);
+                    l += tsum;
                 } else {
                     // ragged tail tile of the chunk: online update per 32-column block with column masks
                     const int nchunks = (((valid + 15) & ~15) + 31) >> 5;
