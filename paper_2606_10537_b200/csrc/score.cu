@@ -17,7 +17,8 @@ namespace pdllm {
 
 namespace {
 
-constexpr int kScoreThreads = 192;        // 4 softmax warps + TMA warp + MMA warp
+constexpr int kScoreThreads = 320;        // 8 softmax warps (two column halves) + TMA warp + MMA warp
+constexpr int kTmaWarp = 8, kMmaWarp = 9;
 constexpr int kMaxChunksPerCta = 64;
 constexpr bool kPolyShare = true;          // MUFU is co-critical with HBM here (538 M ex2 per C4 launch): offload 1/4
 
@@ -55,6 +56,7 @@ score_kernel(const ScoreParams p, const __grid_constant__ CUtensorMap tmap128, c
     __shared__ uint64_t bars[2 * ST + 4];   // k_full[ST], k_free[ST], s_ready[2], s_free[2]
     __shared__ uint32_t tmem_slot;
     __shared__ float s_acc[kMaxChunksPerCta * 4];
+    __shared__ float s_ml[2][kTileM][2];      // column half 1's (m_ref, l) per row, double-buffered by chunk parity
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int group = blockIdx.x / p.m_tiles, mt = blockIdx.x % p.m_tiles, bg = blockIdx.y;
@@ -70,12 +72,12 @@ score_kernel(const ScoreParams p, const __grid_constant__ CUtensorMap tmap128, c
 
     if (tid == 0) {
         for (int s = 0; s < ST; ++s) { mbar_init(k_full(s), 1); mbar_init(k_free(s), 1); }
-        for (int i = 0; i < 2; ++i) { mbar_init(s_ready(i), 1); mbar_init(s_free(i), 128); }
+        for (int i = 0; i < 2; ++i) { mbar_init(s_ready(i), 1); mbar_init(s_free(i), 256); }
         fence_mbar_init();
         tma_prefetch_desc(&tmap128);
         tma_prefetch_desc(&tmap16);
     }
-    if (warp == 5) {
+    if (warp == kMmaWarp) {
         tmem_alloc(smem_u32(&tmem_slot), 256);
         tmem_relinquish();
     }
@@ -97,7 +99,7 @@ score_kernel(const ScoreParams p, const __grid_constant__ CUtensorMap tmap128, c
     tc_fence_after();
     const uint32_t tmem = tmem_slot;
 
-    if (warp == 4) {
+    if (warp == kTmaWarp) {
         // =============================== TMA producer ===============================
         if (lane == 0) {
             const uint64_t policy = l2_policy_evict_first();
@@ -123,7 +125,7 @@ score_kernel(const ScoreParams p, const __grid_constant__ CUtensorMap tmap128, c
             }
         }
         __syncwarp();
-    } else if (warp == 5) {
+    } else if (warp == kMmaWarp) {
         // =============================== MMA issuer ===============================
         if (lane == 0) {
             int q = 0;
@@ -153,8 +155,11 @@ score_kernel(const ScoreParams p, const __grid_constant__ CUtensorMap tmap128, c
         // Per chunk a running (reference max m_ref, sum l) in log2 units.  The chunk's first tile fixes m_ref with a max
         // pass; later tiles take one exp pass against it.  A 32-column block whose row sum exceeds kSumLimit (some
         // logit outgrew the reference by > 13 octaves; rare) raises m_ref by whole octaves and is recomputed.
-        const uint32_t lane_base = (uint32_t)(warp * 32) << 16;
-        const bool row_ok = mt * kTileM + tid < p.rows;
+        // Two threads per row: warps 0-3 take columns 0-63 of every tile, warps 4-7 columns 64-127 (both may read
+        // the row's TMEM lanes), each with its own (m_ref, l); the halves are merged once per chunk.
+        const int half = warp >> 2, row = tid & (kTileM - 1);
+        const uint32_t lane_base = ((uint32_t)((warp & 3) * 32) << 16) + 64u * (uint32_t)half;
+        const bool row_ok = mt * kTileM + row < p.rows;
         constexpr float kSumLimit = 8192.f;
         int q = 0;
         for (int n = n0; n < n1; ++n) {
@@ -195,15 +200,12 @@ score_kernel(const ScoreParams p, const __grid_constant__ CUtensorMap tmap128, c
                     for (;;) {
                         if (max_pass) {
                             float mx[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
-#pragma unroll 1
-                            for (int h = 0; h < 2; ++h) {
-                                tmem_ld32(tS + 64u * h, va);
-                                tmem_ld32(tS + 64u * h + 32u, vb);
-                                tmem_wait_ld();
+                            tmem_ld32(tS, va);
+                            tmem_ld32(tS + 32u, vb);
+                            tmem_wait_ld();
 #pragma unroll
-                                for (int e = 0; e < 32; ++e)
-                                    mx[e & 3] = fmaxf(mx[e & 3], fmaxf(__uint_as_float(va[e]), __uint_as_float(vb[e])));
-                            }
+                            for (int e = 0; e < 32; ++e)
+                                mx[e & 3] = fmaxf(mx[e & 3], fmaxf(__uint_as_float(va[e]), __uint_as_float(vb[e])));
                             const float tm2 = fmaxf(fmaxf(mx[0], mx[1]), fmaxf(mx[2], mx[3])) * p.c2;
                             if (tt == 0) {
                                 m_ref = tm2;
@@ -213,21 +215,15 @@ score_kernel(const ScoreParams p, const __grid_constant__ CUtensorMap tmap128, c
                                 m_ref += up;
                             }
                         }
-                        // TMEM loads one block ahead of the arithmetic
+                        // this thread's 64 columns; the second TMEM load flies under the first block's arithmetic
                         tmem_ld32(tS, va);
                         tmem_wait_ld();
                         tmem_ld32(tS + 32u, vb);
                         tsum = block_sum(va);
                         tmem_wait_ld();
-                        tmem_ld32(tS + 64u, va);
-                        tsum += block_sum(vb);
-                        tmem_wait_ld();
-                        tmem_ld32(tS + 96u, vb);
-                        tsum += block_sum(va);
-                        tmem_wait_ld();
                         tsum += block_sum(vb);
                         // some logit outgrew the reference by > 13 octaves (rare): redo the tile behind a max pass
-                        if (!__any_sync(0xffffffffu, !(tsum <= 4.f * kSumLimit))) break;
+                        if (!__any_sync(0xffffffffu, !(tsum <= 2.f * kSumLimit))) break;
                         max_pass = true;
                     }
                     tc_fence_before();
@@ -235,7 +231,12 @@ score_kernel(const ScoreParams p, const __grid_constant__ CUtensorMap tmap128, c
                     l += tsum;
                 } else {
                     // ragged tail tile of the chunk: online update per 32-column block with column masks
-                    const int nchunks = (((valid + 15) & ~15) + 31) >> 5;
+                    const int mine = max(0, min(64, valid - 64 * half));       // valid columns of this thread's half
+                    const int nchunks = (mine + 31) >> 5;
+                    if (nchunks == 0) {
+                        tc_fence_before();
+                        mbar_arrive(s_free(buf));
+                    }
                     for (int ch = 0; ch < nchunks; ++ch) {
                         uint32_t v[32];
                         tmem_ld32(tS + 32u * ch, v);
@@ -244,7 +245,7 @@ score_kernel(const ScoreParams p, const __grid_constant__ CUtensorMap tmap128, c
                             tc_fence_before();
                             mbar_arrive(s_free(buf));
                         }
-                        const int nv = valid - ch * 32;
+                        const int nv = mine - ch * 32;
                         float cmax = -INFINITY;
 #pragma unroll
                         for (int e = 0; e < 32; ++e)
@@ -259,16 +260,27 @@ score_kernel(const ScoreParams p, const __grid_constant__ CUtensorMap tmap128, c
                     }
                 }
             }
-            // chunk n finished: log-mass of this row, summed over the tile's rows (fixed order)
-            float ell = row_ok ? (m_ref + lg2_approx(l)) * 0.6931471805599453f : 0.f;
+            // chunk n finished: merge the two column halves, then the log-mass of this row, summed over the tile's rows
+            float(*ml)[2] = s_ml[(n - n0) & 1];
+            if (half == 1) {
+                ml[row][0] = m_ref;
+                ml[row][1] = l;
+            }
+            asm volatile("bar.sync 1, 256;" ::: "memory");
+            if (half == 0) {
+                const float m1 = ml[row][0], l1 = ml[row][1];
+                const float m = fmaxf(m_ref, m1);
+                const float lt = l * ex2_approx(m_ref - m) + (l1 > 0.f ? l1 * ex2_approx(m1 - m) : 0.f);
+                float ell = row_ok ? (m + lg2_approx(lt)) * 0.6931471805599453f : 0.f;
 #pragma unroll
-            for (int o = 16; o > 0; o >>= 1) ell += __shfl_xor_sync(0xffffffffu, ell, o);
-            if (lane == 0) s_acc[(n - n0) * 4 + warp] = ell;
+                for (int o = 16; o > 0; o >>= 1) ell += __shfl_xor_sync(0xffffffffu, ell, o);
+                if (lane == 0) s_acc[(n - n0) * 4 + warp] = ell;
+            }
         }
     }
     tc_fence_before();
     __syncthreads();
-    if (warp == 5) tmem_dealloc(tmem, 256);
+    if (warp == kMmaWarp) tmem_dealloc(tmem, 256);
     if (tid < n1 - n0) {
         const float tot = ((s_acc[tid * 4 + 0] + s_acc[tid * 4 + 1]) + (s_acc[tid * 4 + 2] + s_acc[tid * 4 + 3])) * p.inv_rows;
         float *dst = p.scores + (int64_t)bg * p.N + n0 + tid;
