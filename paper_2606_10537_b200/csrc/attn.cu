@@ -393,60 +393,60 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
             uint32_t lq = lq_base;                        // mode B: loads are consumed strictly in ring order
             auto tile_of = [&](int s, int j) { return it.modeA ? it.t0 + j : it.t0 + 2 * j + s; };
             auto n_mma_of = [&](int tile) { return (uint32_t)((min(kTileN, p.S_kv - tile * kTileN) + 15) & ~15); };
-            auto issue_qk = [&](int s, int j) {
-                const int tile = tile_of(s, j);
+            // the eight SS MMAs of S_s = Q_s K^T and their commits (call from the elected lane only)
+            auto emit_qk = [&](int s, int tile, int slot, bool release) {
+                const uint32_t a_lo = lo_k | ((sQ(it.modeA ? s : 0) & 0x3FFFFu) >> 4);
+                const uint32_t b_lo = lo_k | ((sKV(slot) & 0x3FFFFu) >> 4);
+                const uint32_t idesc = umma_idesc_bf16(kTileM, n_mma_of(tile), 0, 0);
+                const uint32_t tS = tmem + 128u * s;
+#pragma unroll
+                for (int ks = 0; ks < D / 16; ++ks) {
+                    // 16 columns = 32 bytes inside the 128-byte swizzle row; next panel every 4 steps
+                    const uint32_t koff = (uint32_t)(((ks >> 2) * Cfg::kPanelBytes + (ks & 3) * 32u) >> 4);
+                    umma_ss_lohi(tS, a_lo + koff, b_lo + koff, hi_k, idesc, ks > 0);
+                }
+                umma_commit(bar(BAR_SREADY0 + s));
+                if (release) umma_commit(kv_free(slot));
+                if (++qk_issued == qk_total) umma_commit(bar(BAR_QFREE));
+            };
+            auto wait_load = [&](uint32_t q) { mbar_wait(kv_full((int)(q % ST)), (q / ST) & 1u); };
+            mbar_wait(bar(BAR_QFULL), (uint32_t)n_done & 1u);
+            for (int s = 0; s < 2; ++s) {                 // prologue: QK(0,0), QK(1,0)
+                if (n_s[s] == 0) continue;
+                const int tile = tile_of(s, 0);
                 const uint32_t q = it.modeA ? lq_base + 2u * (uint32_t)(tile - it.t0) : lq++;
-                const int slot = (int)(q % ST);
-                const bool release = !it.modeA || s == 1;     // last user of this K tile
-                if (lane == 0) PDLLM_TR(20, s);
                 if (!it.modeA || s == 0) {
-                    mbar_wait(kv_full(slot), (q / ST) & 1u);
+                    wait_load(q);
                     fence_proxy_async_smem();             // cp.async (generic proxy) wrote the tile
                 }
                 tc_fence_after();
-                const bool last_qk = ++qk_issued == qk_total;
-                if (elect_one()) {
-                    const uint32_t a_lo = lo_k | ((sQ(it.modeA ? s : 0) & 0x3FFFFu) >> 4);
-                    const uint32_t b_lo = lo_k | ((sKV(slot) & 0x3FFFFu) >> 4);
-                    const uint32_t idesc = umma_idesc_bf16(kTileM, n_mma_of(tile), 0, 0);
-                    const uint32_t tS = tmem + 128u * s;
-#pragma unroll
-                    for (int ks = 0; ks < D / 16; ++ks) {
-                        // 16 columns = 32 bytes inside the 128-byte swizzle row; next panel every 4 steps
-                        const uint32_t koff = (uint32_t)(((ks >> 2) * Cfg::kPanelBytes + (ks & 3) * 32u) >> 4);
-                        umma_ss_lohi(tS, a_lo + koff, b_lo + koff, hi_k, idesc, ks > 0);
-                    }
-                    umma_commit(bar(BAR_SREADY0 + s));
-                    if (release) umma_commit(kv_free(slot));
-                    if (last_qk) umma_commit(bar(BAR_QFREE));
-                }
+                if (elect_one()) emit_qk(s, tile, (int)(q % ST), !it.modeA || s == 1);
                 __syncwarp();
-                if (lane == 0) PDLLM_TR(22, s);
-            };
-            mbar_wait(bar(BAR_QFULL), (uint32_t)n_done & 1u);
-            issue_qk(0, 0);
-            if (n_s[1] > 0) issue_qk(1, 0);
+            }
             for (int j = 0; j < n_s[0]; ++j) {
                 for (int s = 0; s < 2; ++s) {
                     if (j >= n_s[s]) continue;
-                    const int tile = tile_of(s, j);
-                    const uint32_t q = it.modeA ? lq_base + 2u * (uint32_t)(tile - it.t0) + 1u : lq++;
-                    const int slot = (int)(q % ST);
-                    const bool release = !it.modeA || s == 1;     // last user of this V tile
-                    if (lane == 0) PDLLM_TR(23, s);
-                    mbar_wait(bar(BAR_PREADY0 + s), n_pready[s]++ & 1u);
-                    if (lane == 0) PDLLM_TR(24, s);
-                    if (j == 0 && n_oready[s] > 0) mbar_wait(bar(BAR_OFREE0 + s), (n_oready[s] - 1) & 1u);
-                    if (!it.modeA || s == 0) {
-                        mbar_wait(kv_full(slot), (q / ST) & 1u);
+                    const bool fresh = !it.modeA || s == 0, release = !it.modeA || s == 1;
+                    const bool has_next = j + 1 < n_s[s], last_pv = !has_next;
+                    const int tile = tile_of(s, j), tile_n = tile_of(s, j + 1);
+                    const uint32_t q_v = it.modeA ? lq_base + 2u * (uint32_t)(tile - it.t0) + 1u : lq++;
+                    const uint32_t q_k = !has_next ? 0u : (it.modeA ? lq_base + 2u * (uint32_t)(tile_n - it.t0) : lq++);
+                    // the loads this stream step needs have normally landed long ago: cross them into the async proxy
+                    // BEFORE waiting for P, so that P*V and the next Q*K^T issue back to back once P is there
+                    if (fresh) {
+                        wait_load(q_v);
+                        if (has_next) wait_load(q_k);
                         fence_proxy_async_smem();
                     }
+                    if (lane == 0) PDLLM_TR(23, s);
+                    mbar_wait(bar(BAR_PREADY0 + s), n_pready[s]++ & 1u);
+                    if (j == 0 && n_oready[s] > 0) mbar_wait(bar(BAR_OFREE0 + s), (n_oready[s] - 1) & 1u);
                     tc_fence_after();
                     if (lane == 0) PDLLM_TR(25, s);
                     const int ksteps = (int)(n_mma_of(tile) >> 4);
-                    const bool last_pv = j == n_s[s] - 1;
                     if (elect_one()) {
                         // 16 kv rows per step: A = 8 TMEM columns of packed bf16 P, B = 16 V rows (MN-major, 2048 B)
+                        const int slot = (int)(q_v % ST);
                         const uint32_t v_lo = lo_v | ((sKV(slot) & 0x3FFFFu) >> 4);
                         const uint32_t tS = tmem + 128u * s, tO = tmem + kOCol + 128u * s;
                         if (ksteps == kTileN / 16) {
@@ -459,11 +459,11 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
                         }
                         if (release) umma_commit(kv_free(slot));
                         if (last_pv) umma_commit(bar(BAR_OREADY0 + s));
+                        if (has_next) emit_qk(s, tile_n, (int)(q_k % ST), release);
                     }
                     __syncwarp();
                     if (last_pv) ++n_oready[s];
                     if (lane == 0) PDLLM_TR(26, s);
-                    if (j + 1 < n_s[s]) issue_qk(s, j + 1);
                 }
             }
             lq_base += 2u * it.nt;
@@ -561,6 +561,7 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
                         }
                         lsum += csum;
                         tmem_st16(tS + 16u * ch, w);
+                        if (row == 0) PDLLM_TR(36, ch);
                     };
                     tmem_ld32(tS, va);
                     tmem_wait_ld();
