@@ -240,3 +240,45 @@ def test_errors(B):
     with pytest.raises(B.PdllmError):                                             # workspace too small for 2 splits
         B.sparse_attn(shape, dev["Q_dec"], dev["Kcache"], dev["Vcache"], dev_i32(inp["planted"]), dev["keep"],
                       dev["K_dec"], dev["V_dec"], n_splits=2, workspace=ws)
+
+
+# --------------------------------------------------------------------------- rare paths of the single-pass softmaxes
+def _ramp_inputs(C, L_q, L_d, H, H_kv, d, gain):
+    """Keys whose logits grow steeply along the cached sequence (each KV tile, and each 32-column block inside a
+    tile, outgrows the running reference max by many octaves): exercises the overflow -> rescale paths."""
+    w, inp = _inputs("tiny", C=C, L_q=L_q, L_d=L_d, H=H, H_kv=H_kv, d=d, keep=1.0)
+    u = np.zeros(w.d, np.float32); u[::2] = 1.0; u /= np.linalg.norm(u)
+    Q = W.bf16_bits_to_f32(inp["Q_dec"]) + 4.0 * u
+    Kc = W.bf16_bits_to_f32(inp["Kcache"]).copy()
+    ramp = np.linspace(0.0, gain, w.N * w.Cp, dtype=np.float32).reshape(w.N, w.Cp, 1)
+    Kc += (20.0 * ramp * u)[None, None]
+    inp["Q_dec"], inp["Kcache"] = W.f32_to_bf16_bits(Q), W.f32_to_bf16_bits(Kc)
+    return w, inp
+
+
+@pytest.mark.parametrize("H,H_kv,L_q,L_d,d", [(4, 4, 64, 64, 64), (8, 2, 64, 64, 128), (2, 2, 100, 284, 128)])
+def test_attn_growing_logits_all_item_kinds(B, H, H_kv, L_q, L_d, d):
+    """pair items (two query tiles share K/V), single items (in-CTA Split-S merge) and GQA packing, each with a
+    reference max that has to be raised inside tiles."""
+    w, inp = _ramp_inputs(C=300, L_q=L_q, L_d=L_d, H=H, H_kv=H_kv, d=d, gain=6.0)
+    _attn_case(B, w, inp, [1, 2, 5])
+
+
+def test_scores_growing_logits(B):
+    """chunk scores when the logits inside every chunk outgrow the chunk's first-tile reference max (redo path)."""
+    w, inp = _ramp_inputs(C=700, L_q=128, L_d=8, H=4, H_kv=4, d=128, gain=40.0)
+    shape = B.Shape.of(w)
+    got = B.score_chunks(shape, dev_bf16(inp["Q_dec"]), dev_bf16(inp["Kcache"]))
+    ref = oracle.scores(inp["Q_dec"], inp["Kcache"], w.L_q)
+    check_close(got, ref, SCORE_ABS * max(1.0, float(np.abs(ref).max()) / 100.0), what="scores (growing logits)")
+    check_exact(B.select_topk(shape, got), oracle.topk(ref, w.K))
+
+
+@pytest.mark.parametrize("kw", [
+    dict(H=4, H_kv=4, d=64, C=500, K=3, keep=1.0, L_q=128, L_d=128),     # d = 64: pair items, 13 KV tiles
+    dict(H=2, H_kv=2, d=128, C=640, K=8, keep=1.0, L_q=32, L_d=32),      # one query tile per group: single items, 41 tiles
+    dict(H=16, H_kv=2, d=128, C=256, K=4, keep=0.3, L_q=48, L_d=80),     # GQA G = 8: 8 query tiles per group
+])
+def test_attn_item_shapes(B, kw):
+    w, inp = _inputs("tiny", **kw)
+    _attn_case(B, w, inp, [0, 1, 3, 7])
