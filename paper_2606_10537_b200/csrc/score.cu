@@ -27,7 +27,8 @@ struct ScoreParams {
     int64_t q_batch_stride, q_head_stride;
     float *scores;
     int H_kv, G, N, Cp, L_q, rows;        // rows = G * L_q
-    int m_tiles, n_groups, cpc;           // chunks per CTA
+    int m_tiles;
+    int64_t units;                        // (b, g, M tile, chunk) work units, split evenly over the persistent CTAs
     float c2, inv_rows;
     int use_atomic, evict_first;
 };
@@ -59,9 +60,8 @@ score_kernel(const ScoreParams p, const __grid_constant__ CUtensorMap tmap128, c
     __shared__ float s_ml[2][kTileM][2];      // column half 1's (m_ref, l) per row, double-buffered by chunk parity
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const int group = blockIdx.x / p.m_tiles, mt = blockIdx.x % p.m_tiles, bg = blockIdx.y;
-    const int b = bg / p.H_kv, g = bg % p.H_kv;
-    const int n0 = group * p.cpc, n1 = min(p.N, n0 + p.cpc);
+    // persistent CTA: a contiguous range of the units u = ((bg * m_tiles + mt) * N + n)
+    const int64_t u_lo = p.units * blockIdx.x / gridDim.x, u_hi = p.units * (blockIdx.x + 1) / gridDim.x;
     const int tiles_per_chunk = (p.Cp + kTileN - 1) / kTileN;
 
     const uint32_t bar0 = smem_u32(&bars[0]);
@@ -81,7 +81,21 @@ score_kernel(const ScoreParams p, const __grid_constant__ CUtensorMap tmap128, c
         tmem_alloc(smem_u32(&tmem_slot), 256);
         tmem_relinquish();
     }
-    // Q tile (scoring rows mt*128.. of group g; row m -> head g*G + m / L_q, position m % L_q)
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem = tmem_slot;
+    int q = 0;                                // tile-step counter of the K ring / S buffers (every role counts alike)
+
+    for (int64_t u = u_lo; u < u_hi;) {
+    // ---- one segment: up to kMaxChunksPerCta consecutive chunks n0..n1-1 of one (bg, M tile)
+    const int64_t bgm = u / p.N;
+    const int n0 = (int)(u - bgm * p.N);
+    const int n1 = (int)min((int64_t)p.N, (int64_t)n0 + min(u_hi - u, (int64_t)kMaxChunksPerCta));
+    const int bg = (int)(bgm / p.m_tiles), mt = (int)(bgm % p.m_tiles);
+    const int b = bg / p.H_kv, g = bg % p.H_kv;
+    // Q tile (scoring rows mt*128.. of group g; row m -> head g*G + m / L_q, position m % L_q); the previous
+    // segment's MMAs are complete (its softmax consumed every S tile before the barrier below was passed)
     for (int i = tid; i < kTileM * kChunksPerRow; i += kScoreThreads) {
         const int r = i / kChunksPerRow, c = i % kChunksPerRow;
         const int m = mt * kTileM + r;
@@ -97,13 +111,11 @@ score_kernel(const ScoreParams p, const __grid_constant__ CUtensorMap tmap128, c
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
-    const uint32_t tmem = tmem_slot;
 
     if (warp == kTmaWarp) {
         // =============================== TMA producer ===============================
         if (lane == 0) {
             const uint64_t policy = l2_policy_evict_first();
-            int q = 0;
             for (int n = n0; n < n1; ++n) {
                 const int64_t row0 = ((int64_t)bg * p.N + n) * p.Cp;
                 for (int tt = 0; tt < tiles_per_chunk; ++tt, ++q) {
@@ -128,7 +140,6 @@ score_kernel(const ScoreParams p, const __grid_constant__ CUtensorMap tmap128, c
     } else if (warp == kMmaWarp) {
         // =============================== MMA issuer ===============================
         if (lane == 0) {
-            int q = 0;
             for (int n = n0; n < n1; ++n) {
                 for (int tt = 0; tt < tiles_per_chunk; ++tt, ++q) {
                     const int stage = q % ST, buf = q & 1;
@@ -161,7 +172,6 @@ score_kernel(const ScoreParams p, const __grid_constant__ CUtensorMap tmap128, c
         const uint32_t lane_base = ((uint32_t)((warp & 3) * 32) << 16) + 64u * (uint32_t)half;
         const bool row_ok = mt * kTileM + row < p.rows;
         constexpr float kSumLimit = 8192.f;
-        int q = 0;
         for (int n = n0; n < n1; ++n) {
             float m_ref = -INFINITY, l = 0.f;
             // sum over 32 columns of 2^(c2*x - m_ref): packed f32x2 arithmetic, exponentials on the MUFU pipe
@@ -280,13 +290,18 @@ score_kernel(const ScoreParams p, const __grid_constant__ CUtensorMap tmap128, c
     }
     tc_fence_before();
     __syncthreads();
-    if (warp == kMmaWarp) tmem_dealloc(tmem, 256);
+    tc_fence_after();
     if (tid < n1 - n0) {
         const float tot = ((s_acc[tid * 4 + 0] + s_acc[tid * 4 + 1]) + (s_acc[tid * 4 + 2] + s_acc[tid * 4 + 3])) * p.inv_rows;
         float *dst = p.scores + (int64_t)bg * p.N + n0 + tid;
         if (p.use_atomic) atomicAdd(dst, tot);
         else *dst = tot;
     }
+    u += n1 - n0;
+    }   // segments
+    tc_fence_before();
+    __syncthreads();
+    if (warp == kMmaWarp) tmem_dealloc(tmem, 256);
 }
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
@@ -323,7 +338,8 @@ cudaError_t launch_score_d(const ScoreParams &p, const CUtensorMap &t128, const 
     using Cfg = ScoreCfg<D>;
     cudaError_t e = cudaFuncSetAttribute(score_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::kSmem);
     if (e != cudaSuccess) return e;
-    dim3 grid((unsigned)(p.n_groups * p.m_tiles), (unsigned)BG, 1);
+    const int64_t slots = 2ll * device_num_sms();          // two CTAs per SM
+    dim3 grid((unsigned)(p.units < slots ? p.units : slots), 1, 1);
     score_kernel<D><<<grid, kScoreThreads, Cfg::kSmem, st>>>(p, t128, t16);
     return cudaGetLastError();
 }
@@ -341,14 +357,7 @@ cudaError_t launch_score(const Dims &s, const void *Q, int64_t q_batch_stride, i
     p.rows = s.G * s.L_q;
     p.m_tiles = (p.rows + kTileM - 1) / kTileM;
     const int BG = s.B * s.H_kv;
-    // chunks per CTA: about six waves of (2 CTAs x SMs) work items, so the tail wave stays small
-    const int64_t units = (int64_t)BG * s.N * p.m_tiles;
-    const int64_t slots = 2ll * device_num_sms();
-    int cpc = (int)((units + slots * 6 - 1) / (slots * 6));
-    cpc = cpc < 1 ? 1 : (cpc > kMaxChunksPerCta ? kMaxChunksPerCta : cpc);
-    if (cpc > s.N) cpc = s.N;
-    p.cpc = cpc;
-    p.n_groups = (s.N + cpc - 1) / cpc;
+    p.units = (int64_t)BG * s.N * p.m_tiles;
     p.c2 = s.scale * 1.4426950408889634f;
     p.inv_rows = 1.0f / (float)p.rows;
     p.use_atomic = p.m_tiles > 1;
