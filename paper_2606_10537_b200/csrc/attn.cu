@@ -166,9 +166,10 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
     auto sQ = [&](int s) { return smem_base + Cfg::kTileBytes * (uint32_t)s; };
-    auto sKV = [&](int slot) { return smem_base + Cfg::kTileBytes * (uint32_t)(2 + slot); };
+    // ring slots 0..ST-1 follow the two Q buffers; slot ST is the SECOND Q BUFFER, lent to the ring by single items
+    auto sKV = [&](int slot) { return smem_base + Cfg::kTileBytes * (uint32_t)(slot == ST ? 1 : 2 + slot); };
 
-    __shared__ uint64_t bars[BAR_KV + 2 * ST];
+    __shared__ uint64_t bars[BAR_KV + 2 * (ST + 1)];
     __shared__ uint32_t tmem_slot;
     __shared__ float s_ml[kSoftmaxThreads][2];            // mode B: stream 1's (m_ref, l) for the in-CTA merge
 
@@ -176,7 +177,7 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
     const uint32_t bar0 = smem_u32(&bars[0]);
     auto bar = [&](int i) { return bar0 + 8u * i; };
     auto kv_full = [&](int slot) { return bar0 + 8u * (BAR_KV + slot); };
-    auto kv_free = [&](int slot) { return bar0 + 8u * (BAR_KV + ST + slot); };
+    auto kv_free = [&](int slot) { return bar0 + 8u * (BAR_KV + ST + 1 + slot); };
 
     if (tid == 0) {
         mbar_init(bar(BAR_QFULL), kProducerThreads);
@@ -187,7 +188,7 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
             mbar_init(bar(BAR_OREADY0 + s), 1);
             mbar_init(bar(BAR_OFREE0 + s), kSoftmaxThreads);
         }
-        for (int s = 0; s < ST; ++s) {
+        for (int s = 0; s <= ST; ++s) {
             mbar_init(kv_full(s), kProducerThreads);
             mbar_init(kv_free(s), 1);
         }
@@ -256,7 +257,10 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
                 if (do_v) cp_async16(dst_v + dst_of(i), reinterpret_cast<const void *>(vrow0_c + o));
             }
         };
-        uint32_t lq = 0;                                  // ring load counter (continues across items)
+        // Ring cursor and per-slot phase bits (continue across items).  Pair items use ST slots, single items ST + 1.
+        // free_bits: parity the next use of a slot waits for on its "free" barrier (1 = passes on a fresh barrier).
+        int cur = 0;
+        uint32_t free_bits = (1u << (ST + 1)) - 1u;
         int n_done = 0;                                   // items finished by this CTA
         PDLLM_TRACE_DECL(0)
         for (int ii = blockIdx.x; ii < p.n_items; ii += gridDim.x, ++n_done) {
@@ -284,7 +288,9 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
             };
             // the item's Q tile(s), once the previous item's Q*K^T are all done
             auto load_q = [&]() {
-                if (n_done > 0) wait_free(bar(BAR_QFREE), (uint32_t)(n_done - 1) & 1u);
+                if (n_done > 0 && it.modeA) wait_free(bar(BAR_QFREE), (uint32_t)(n_done - 1) & 1u);
+                // a pair item writes the second Q buffer: the last K/V tile a single item parked there must be released
+                if (it.modeA) wait_free(kv_free(ST), (free_bits >> ST) & 1u);
                 const uint16_t *Qg = p.Q + bg * p.rows_g * D;
                 const int n_q = it.modeA ? 2 : 1;
                 for (int s = 0; s < n_q; ++s) {
@@ -308,8 +314,16 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
                 const uint16_t *base = in_cache ? (is_v ? Vc : Kc) : (is_v ? Vd : Kd);
                 return reinterpret_cast<uint64_t>(base + row_off);
             };
-            auto wait_slot = [&](uint32_t q) {
-                if (q >= (uint32_t)ST) wait_free(kv_free((int)(q % ST)), ((q / ST) - 1) & 1u);
+            const int n_slots = it.modeA ? ST : ST + 1;
+            if (it.modeA && cur == ST) cur = 0;
+            // a single item may drop a tile into the second Q buffer right away: the previous item's Q*K^T must be done
+            if (!it.modeA && n_done > 0) wait_free(bar(BAR_QFREE), (uint32_t)(n_done - 1) & 1u);
+            auto take_slot = [&]() {                      // next ring slot, once its previous tile has been released
+                const int sl = cur;
+                wait_free(kv_free(sl), (free_bits >> sl) & 1u);
+                free_bits ^= 1u << sl;
+                cur = cur + 1 == n_slots ? 0 : cur + 1;
+                return sl;
             };
             // K and/or V rows of one tile into the given slots
             const uint64_t kbase_c = reinterpret_cast<uint64_t>(Kc + c * 8), vbase_c = reinterpret_cast<uint64_t>(Vc + c * 8);
@@ -328,31 +342,29 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
             if (it.modeA) {
                 // tile by tile, K and V together (one index computation, one cp.async group): loads 2*jt and 2*jt + 1
                 prefetch_index(it.t0);
-                for (int jt = 0; jt < it.nt; ++jt, lq += 2) {
+                for (int jt = 0; jt < it.nt; ++jt) {
                     const int my_idx = nx_base + nx_raw;
-                    if (pt == 0) PDLLM_TR(10, lq);
+                    if (pt == 0) PDLLM_TR(10, jt);
                     if (jt + 1 < it.nt) prefetch_index(it.t0 + jt + 1);         // in flight while this tile is issued
-                    wait_slot(lq);
-                    wait_slot(lq + 1);
-                    if (pt == 0) PDLLM_TR(11, lq);
-                    load_tile(it.t0 + jt, my_idx, sKV((int)(lq % ST)), sKV((int)((lq + 1) % ST)), true, true);
-                    if (pt == 0) PDLLM_TR(12, lq);
-                    publish(kv_full((int)(lq % ST)));
-                    publish(kv_full((int)((lq + 1) % ST)));
+                    const int slot_k = take_slot(), slot_v = take_slot();
+                    if (pt == 0) PDLLM_TR(11, jt);
+                    load_tile(it.t0 + jt, my_idx, sKV(slot_k), sKV(slot_v), true, true);
+                    if (pt == 0) PDLLM_TR(12, jt);
+                    publish(kv_full(slot_k));
+                    publish(kv_full(slot_v));
                     if (jt == 0) load_q();
                 }
             } else {
                 // one tile per load, in the MMA warp's consumption order K(t0); { K(t0+i+1), V(t0+i) }; V(t0+nt-1)
                 // (each tile has a single user); a tile's indices are computed once and serve its K and its V load
                 auto load_one = [&](int tile, int idx, bool is_v) {
-                    if (pt == 0) PDLLM_TR(10, lq);
-                    wait_slot(lq);
-                    if (pt == 0) PDLLM_TR(11, lq);
-                    const uint32_t dst = sKV((int)(lq % ST));
+                    if (pt == 0) PDLLM_TR(10, tile);
+                    const int slot = take_slot();
+                    if (pt == 0) PDLLM_TR(11, tile);
+                    const uint32_t dst = sKV(slot);
                     load_tile(tile, idx, dst, dst, !is_v, is_v);
-                    if (pt == 0) PDLLM_TR(12, lq);
-                    publish(kv_full((int)(lq % ST)));
-                    ++lq;
+                    if (pt == 0) PDLLM_TR(12, tile);
+                    publish(kv_full(slot));
                 };
                 prefetch_index(it.t0);
                 int idx_cur = nx_base + nx_raw;
@@ -377,7 +389,8 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
         // under the other stream's MMAs).  The warp stays converged (all lanes wait on the barriers); one elected
         // lane issues the tcgen05 instructions, so the descriptors stay in uniform registers.
         PDLLM_TRACE_DECL(1)
-        uint32_t lq_base = 0;
+        int cur = 0;                                      // ring cursor / phase bits, mirrored from the producers
+        uint32_t full_bits = 0u;
         uint32_t n_pready[2] = {0, 0}, n_oready[2] = {0, 0};
         int n_done = 0;
         constexpr uint32_t idesc_pv = umma_idesc_bf16(kTileM, D, 0, 1);
@@ -390,7 +403,16 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
             const int n_s[2] = {it.modeA ? it.nt : (it.nt + 1) / 2, it.modeA ? it.nt : it.nt / 2};
             const int qk_total = n_s[0] + n_s[1];
             int qk_issued = 0;
-            uint32_t lq = lq_base;                        // mode B: loads are consumed strictly in ring order
+            const int n_slots = it.modeA ? ST : ST + 1;
+            if (it.modeA && cur == ST) cur = 0;
+            int k_slot = 0, v_slot = 0;                   // pair items: the tile both streams are on
+            auto next_load = [&]() {                      // wait for the next tile of the ring (loads are consumed in order)
+                const int sl = cur;
+                mbar_wait(kv_full(sl), (full_bits >> sl) & 1u);
+                full_bits ^= 1u << sl;
+                cur = cur + 1 == n_slots ? 0 : cur + 1;
+                return sl;
+            };
             auto tile_of = [&](int s, int j) { return it.modeA ? it.t0 + j : it.t0 + 2 * j + s; };
             auto n_mma_of = [&](int tile) { return (uint32_t)((min(kTileN, p.S_kv - tile * kTileN) + 15) & ~15); };
             // the eight SS MMAs of S_s = Q_s K^T and their commits (call from the elected lane only)
@@ -409,18 +431,16 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
                 if (release) umma_commit(kv_free(slot));
                 if (++qk_issued == qk_total) umma_commit(bar(BAR_QFREE));
             };
-            auto wait_load = [&](uint32_t q) { mbar_wait(kv_full((int)(q % ST)), (q / ST) & 1u); };
             mbar_wait(bar(BAR_QFULL), (uint32_t)n_done & 1u);
             for (int s = 0; s < 2; ++s) {                 // prologue: QK(0,0), QK(1,0)
                 if (n_s[s] == 0) continue;
                 const int tile = tile_of(s, 0);
-                const uint32_t q = it.modeA ? lq_base + 2u * (uint32_t)(tile - it.t0) : lq++;
                 if (!it.modeA || s == 0) {
-                    wait_load(q);
+                    k_slot = next_load();
                     fence_proxy_async_smem();             // cp.async (generic proxy) wrote the tile
                 }
                 tc_fence_after();
-                if (elect_one()) emit_qk(s, tile, (int)(q % ST), !it.modeA || s == 1);
+                if (elect_one()) emit_qk(s, tile, k_slot, !it.modeA || s == 1);
                 __syncwarp();
             }
             for (int j = 0; j < n_s[0]; ++j) {
@@ -429,13 +449,11 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
                     const bool fresh = !it.modeA || s == 0, release = !it.modeA || s == 1;
                     const bool has_next = j + 1 < n_s[s], last_pv = !has_next;
                     const int tile = tile_of(s, j), tile_n = tile_of(s, j + 1);
-                    const uint32_t q_v = it.modeA ? lq_base + 2u * (uint32_t)(tile - it.t0) + 1u : lq++;
-                    const uint32_t q_k = !has_next ? 0u : (it.modeA ? lq_base + 2u * (uint32_t)(tile_n - it.t0) : lq++);
                     // the loads this stream step needs have normally landed long ago: cross them into the async proxy
                     // BEFORE waiting for P, so that P*V and the next Q*K^T issue back to back once P is there
                     if (fresh) {
-                        wait_load(q_v);
-                        if (has_next) wait_load(q_k);
+                        v_slot = next_load();
+                        if (has_next) k_slot = next_load();
                         fence_proxy_async_smem();
                     }
                     if (lane == 0) PDLLM_TR(23, s);
@@ -446,7 +464,7 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
                     const int ksteps = (int)(n_mma_of(tile) >> 4);
                     if (elect_one()) {
                         // 16 kv rows per step: A = 8 TMEM columns of packed bf16 P, B = 16 V rows (MN-major, 2048 B)
-                        const int slot = (int)(q_v % ST);
+                        const int slot = v_slot;
                         const uint32_t v_lo = lo_v | ((sKV(slot) & 0x3FFFFu) >> 4);
                         const uint32_t tS = tmem + 128u * s, tO = tmem + kOCol + 128u * s;
                         if (ksteps == kTileN / 16) {
@@ -459,14 +477,13 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
                         }
                         if (release) umma_commit(kv_free(slot));
                         if (last_pv) umma_commit(bar(BAR_OREADY0 + s));
-                        if (has_next) emit_qk(s, tile_n, (int)(q_k % ST), release);
+                        if (has_next) emit_qk(s, tile_n, k_slot, release);
                     }
                     __syncwarp();
                     if (last_pv) ++n_oready[s];
                     if (lane == 0) PDLLM_TR(26, s);
                 }
             }
-            lq_base += 2u * it.nt;
         }
     } else {
         // =============================== softmax streams (thread = query row) ===============================
