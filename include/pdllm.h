@@ -86,8 +86,9 @@ const char *pdllm_strerror(int status);        /* static string, never NULL */
 int32_t pdllm_auto_splits(const pdllm_shape *shape, int32_t num_sms);
 
 /* Bytes of scratch pdllm_sparse_attn / pdllm_step need for n_splits splits
- * (n_splits == 0: the auto choice for num_sms).  0 when no scratch is needed.
- * Returns 0 for an invalid shape. */
+ * (n_splits == 0: the auto choice for num_sms): always >= 256 (the persistent
+ * attention kernel's work-item counter, cleared by the call itself), plus the fp32
+ * partials when there is more than one split.  Returns 0 for an invalid shape. */
 size_t pdllm_workspace_bytes(const pdllm_shape *shape, int32_t n_splits, int32_t num_sms);
 
 /* Bytes of device scratch pdllm_step_host needs (staging of the per-step tensors
@@ -135,7 +136,7 @@ int pdllm_gather_idx(const pdllm_shape *shape, const int32_t *chunk_ids,
  *   O       device bf16 [B,H,L,d] (out);  LSE device fp32 [B,H,L] (out)
  *   gather_idx_out  device int32 [B,H_kv,K*Bk] (out) or NULL
  *   workspace  device scratch of >= pdllm_workspace_bytes(shape, n_splits, num_sms) bytes
- *              (may be NULL when that is 0)                                        */
+ *              (required; its contents need no initialisation)                     */
 int pdllm_sparse_attn(const pdllm_shape *shape, const void *Q_dec, const void *Kcache,
                       const void *Vcache, const int32_t *chunk_ids, const int32_t *token_keep_idx,
                       const void *K_dec, const void *V_dec, int32_t n_splits,

@@ -62,6 +62,7 @@ struct AttnParams {
     int n_splits, n_tiles;                                // KV tiles of the whole sequence
     int n_qt, n_pairs, n_single;                          // query tiles per group: n_qt = 2*n_pairs + n_single
     int n_pair_items, n_items;
+    int32_t *work_counter;                                // zeroed before launch: next work item to hand out
     int64_t total_rows;                                   // B*H*L
     float c2;                                             // scale * log2(e)
 };
@@ -102,7 +103,7 @@ struct AttnCfg {
 };
 
 // barrier indices (kv_full / kv_free follow)
-enum { BAR_QFULL = 0, BAR_QFREE, BAR_SREADY0, BAR_SREADY1, BAR_PREADY0, BAR_PREADY1, BAR_OREADY0, BAR_OREADY1,
+enum { BAR_ITEM0 = 0, BAR_ITEM1, BAR_ITEM2, BAR_ITEM3, BAR_QFULL, BAR_QFREE, BAR_SREADY0, BAR_SREADY1, BAR_PREADY0, BAR_PREADY1, BAR_OREADY0, BAR_OREADY1,
        BAR_OFREE0, BAR_OFREE1, BAR_KV };
 
 // D[tmem] (+)= A[smem] * B[smem] with the descriptors given as (low word, constant high word)
@@ -171,6 +172,7 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
 
     __shared__ uint64_t bars[BAR_KV + 2 * (ST + 1)];
     __shared__ uint32_t tmem_slot;
+    __shared__ int32_t s_items[4];                        // the CTA's next work items (ring, published by the producers)
     __shared__ float s_ml[kSoftmaxThreads][2];            // mode B: stream 1's (m_ref, l) for the in-CTA merge
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -180,6 +182,7 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
     auto kv_free = [&](int slot) { return bar0 + 8u * (BAR_KV + ST + 1 + slot); };
 
     if (tid == 0) {
+        for (int i = 0; i < 4; ++i) mbar_init(bar(BAR_ITEM0 + i), 1);
         mbar_init(bar(BAR_QFULL), kProducerThreads);
         mbar_init(bar(BAR_QFREE), 1);
         for (int s = 0; s < 2; ++s) {
@@ -263,7 +266,17 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
         uint32_t free_bits = (1u << (ST + 1)) - 1u;
         int n_done = 0;                                   // items finished by this CTA
         PDLLM_TRACE_DECL(0)
-        for (int ii = blockIdx.x; ii < p.n_items; ii += gridDim.x, ++n_done) {
+        // Work items are handed out dynamically (costliest first: pair items, then single items), so CTAs that
+        // finish early take more; thread 0 of the producers fetches, the other roles follow through s_items.
+        for (;; ++n_done) {
+            if (pt == 0) {
+                const int nxt = atomicAdd(p.work_counter, 1);
+                s_items[n_done & 3] = nxt < p.n_items ? nxt : -1;
+            }
+            asm volatile("bar.sync 1, 128;" ::: "memory");
+            const int ii = s_items[n_done & 3];
+            if (pt == 0) mbar_arrive(bar(BAR_ITEM0 + (n_done & 3)));
+            if (ii < 0) break;
             const Item it = decode_item(p, ii);
             const int64_t bg = it.bg;
             const uint16_t *Kc = p.Kc + bg * p.N * p.Cp * D, *Vc = p.Vc + bg * p.N * p.Cp * D;
@@ -398,7 +411,10 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
         const uint32_t hi_k = (uint32_t)(umma_desc_sw128(0, 16, 1024) >> 32);
         const uint32_t hi_v = (uint32_t)(umma_desc_sw128(0, Cfg::kPanelBytes, 1024) >> 32);
         const uint32_t lo_k = (uint32_t)umma_desc_sw128(0, 16, 1024), lo_v = (uint32_t)umma_desc_sw128(0, Cfg::kPanelBytes, 1024);
-        for (int ii = blockIdx.x; ii < p.n_items; ii += gridDim.x, ++n_done) {
+        for (;; ++n_done) {
+            mbar_wait(bar(BAR_ITEM0 + (n_done & 3)), (uint32_t)(n_done >> 2) & 1u);
+            const int ii = s_items[n_done & 3];
+            if (ii < 0) break;
             const Item it = decode_item(p, ii);
             const int n_s[2] = {it.modeA ? it.nt : (it.nt + 1) / 2, it.modeA ? it.nt : it.nt / 2};
             const int qk_total = n_s[0] + n_s[1];
@@ -494,7 +510,10 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
         uint32_t n_sready = 0, n_oready = 0;
         int n_modeB = 0;
         PDLLM_TRACE_DECL(2 + s)
-        for (int ii = blockIdx.x; ii < p.n_items; ii += gridDim.x) {
+        for (int n_done = 0;; ++n_done) {
+            mbar_wait(bar(BAR_ITEM0 + (n_done & 3)), (uint32_t)(n_done >> 2) & 1u);
+            const int ii = s_items[n_done & 3];
+            if (ii < 0) break;
             const Item it = decode_item(p, ii);
             const int n_mine = it.modeA ? it.nt : (s == 0 ? (it.nt + 1) / 2 : it.nt / 2);
             float m_ref = -INFINITY, l = 0.f;
@@ -746,7 +765,7 @@ cudaError_t launch_attn_d(const AttnParams &p, cudaStream_t st) {
 
 cudaError_t launch_attn(const Dims &s, const void *Q_dec, const void *Kcache, const void *Vcache, const int32_t *chunk_ids,
                         const int32_t *keep, const void *K_dec, const void *V_dec, int n_splits, void *O, float *LSE,
-                        float *O_part, float *lse_part, cudaStream_t st) {
+                        float *O_part, float *lse_part, int32_t *work_counter, cudaStream_t st) {
     AttnParams p;
     p.Q = static_cast<const uint16_t *>(Q_dec);
     p.Kc = static_cast<const uint16_t *>(Kcache);
@@ -759,6 +778,7 @@ cudaError_t launch_attn(const Dims &s, const void *Q_dec, const void *Kcache, co
     p.LSE = LSE;
     p.O_part = O_part;
     p.lse_part = lse_part;
+    p.work_counter = work_counter;
     p.N = s.N; p.Cp = s.Cp; p.K = s.K; p.Bk = s.Bk; p.L_s = s.L_s;
     p.S_pre = s.S_pre; p.S_kv = s.S_kv; p.rows_g = s.rows_g;
     p.n_tiles = (s.S_kv + kTileN - 1) / kTileN;

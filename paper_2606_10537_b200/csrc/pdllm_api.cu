@@ -97,10 +97,13 @@ int effective_splits(const Dims &d, int n_splits, int num_sms) {
     return S > T ? T : S;       // no empty split (R10)
 }
 
+// scratch of the attention: 256 bytes for the work-item counter of the persistent kernel (always), then, for S > 1,
+// the fp32 partials O_part [S, rows, d] and lse_part [S, rows]
+constexpr size_t kCounterBytes = 256;
 size_t workspace_for(const Dims &d, int S) {
-    if (S <= 1) return 0;
+    if (S <= 1) return kCounterBytes;
     const size_t rows = (size_t)d.B * d.H * d.L;
-    return align_up((size_t)S * rows * d.d * sizeof(float), 256) + align_up((size_t)S * rows * sizeof(float), 256);
+    return kCounterBytes + align_up((size_t)S * rows * d.d * sizeof(float), 256) + align_up((size_t)S * rows * sizeof(float), 256);
 }
 
 struct HostScratch {
@@ -213,17 +216,21 @@ int record(void *ev, cudaStream_t st) {
 // a3 + a4 + a5 on validated arguments; ev_mid / ev_end (may be NULL) are recorded after a4 / a5.
 int attn_impl(const Dims &d, const void *Q_dec, const void *Kcache, const void *Vcache, const int32_t *chunk_ids,
               const int32_t *token_keep_idx, const void *K_dec, const void *V_dec, int S, void *O, float *LSE,
-              int32_t *gather_idx_out, void *workspace, void *ev_mid, void *ev_end, cudaStream_t st) {
+              int32_t *gather_idx_out, void *workspace, bool counter_zeroed, void *ev_mid, void *ev_end, cudaStream_t st) {
+    int32_t *counter = static_cast<int32_t *>(workspace);
+    if (!counter_zeroed)
+        if (int rc = cuda_rc(cudaMemsetAsync(counter, 0, sizeof(int32_t), st))) return rc;
     if (gather_idx_out)
         if (int rc = cuda_rc(launch_gather_idx(d, chunk_ids, token_keep_idx, gather_idx_out, st))) return rc;
     const size_t rows = (size_t)d.B * d.H * d.L;
     float *O_part = nullptr, *lse_part = nullptr;
     if (S > 1) {
-        O_part = static_cast<float *>(workspace);
-        lse_part = reinterpret_cast<float *>(static_cast<char *>(workspace) + align_up((size_t)S * rows * d.d * sizeof(float), 256));
+        O_part = reinterpret_cast<float *>(static_cast<char *>(workspace) + kCounterBytes);
+        lse_part = reinterpret_cast<float *>(static_cast<char *>(workspace) + kCounterBytes +
+                                             align_up((size_t)S * rows * d.d * sizeof(float), 256));
     }
     if (int rc = cuda_rc(launch_attn(d, Q_dec, Kcache, Vcache, chunk_ids, token_keep_idx, K_dec, V_dec, S, O, LSE, O_part,
-                                     lse_part, st)))
+                                     lse_part, counter, st)))
         return rc;
     if (int rc = record(ev_mid, st)) return rc;
     if (S > 1)
@@ -242,7 +249,7 @@ int attn_validate(const pdllm_shape *shape, const void *Q_dec, const void *Kcach
         return PDLLM_ERR_ALIGN;
     *S = effective_splits(*d, n_splits, device_num_sms());
     const size_t need = workspace_for(*d, *S);
-    if (need > 0 && (!workspace || workspace_bytes < need)) return PDLLM_ERR_WORKSPACE;
+    if (!workspace || workspace_bytes < need) return PDLLM_ERR_WORKSPACE;
     return PDLLM_OK;
 }
 
@@ -258,7 +265,7 @@ int pdllm_sparse_attn(const pdllm_shape *shape, const void *Q_dec, const void *K
                                workspace, workspace_bytes, &d, &S))
         return rc;
     return attn_impl(d, Q_dec, Kcache, Vcache, chunk_ids, token_keep_idx, K_dec, V_dec, S, O, LSE, gather_idx_out,
-                     workspace, nullptr, nullptr, static_cast<cudaStream_t>(stream));
+                     workspace, false, nullptr, nullptr, static_cast<cudaStream_t>(stream));
 }
 
 int pdllm_step_profiled(const pdllm_shape *shape, const void *Q_dec, const void *Kcache, const void *Vcache,
@@ -275,6 +282,8 @@ int pdllm_step_profiled(const pdllm_shape *shape, const void *Q_dec, const void 
         return rc;
     if (!aligned16(scores_out)) return PDLLM_ERR_ALIGN;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
+    // the attention's work-item counter is cleared here, far ahead of its kernel (off the step's critical path)
+    if (int rc = cuda_rc(cudaMemsetAsync(workspace, 0, sizeof(int32_t), st))) return rc;
     if (int rc = record(ev ? ev->begin : nullptr, st)) return rc;
     if (int rc = cuda_rc(launch_score(d, Q_dec, (int64_t)d.H * d.L * d.d, (int64_t)d.L * d.d, Kcache, scores_out, st)))
         return rc;
@@ -282,7 +291,7 @@ int pdllm_step_profiled(const pdllm_shape *shape, const void *Q_dec, const void 
     if (int rc = cuda_rc(launch_topk(d, scores_out, chunk_ids_out, st))) return rc;
     if (int rc = record(ev ? ev->after_topk : nullptr, st)) return rc;
     return attn_impl(d, Q_dec, Kcache, Vcache, chunk_ids_out, token_keep_idx, K_dec, V_dec, S, O, LSE, gather_idx_out,
-                     workspace, ev ? ev->after_attn : nullptr, ev ? ev->end : nullptr, st);
+                     workspace, true, ev ? ev->after_attn : nullptr, ev ? ev->end : nullptr, st);
 }
 
 int pdllm_step(const pdllm_shape *shape, const void *Q_dec, const void *Kcache, const void *Vcache,

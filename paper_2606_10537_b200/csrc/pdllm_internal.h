@@ -36,7 +36,7 @@ cudaError_t launch_score(const Dims &s, const void *Q, int64_t q_batch_stride, i
 // ---- a3+a4 (+a5 when n_splits > 1)
 cudaError_t launch_attn(const Dims &s, const void *Q_dec, const void *Kcache, const void *Vcache, const int32_t *chunk_ids,
                         const int32_t *keep, const void *K_dec, const void *V_dec, int n_splits, void *O, float *LSE,
-                        float *O_part, float *lse_part, cudaStream_t st);
+                        float *O_part, float *lse_part, int32_t *work_counter, cudaStream_t st);
 
 int device_num_sms();
 

@@ -45,10 +45,10 @@ def test_auto_splits(name, expect_min, expect_max):
 def test_workspace_bytes():
     w = W.CONFIGS["sparse32k"]
     sh = B.Shape.of(w)
-    assert B.workspace_bytes(sh, 1, 148) == 0
+    assert B.workspace_bytes(sh, 1, 148) == 256          # the persistent kernel's work-item counter
     rows = w.B * w.H * w.L
     got = B.workspace_bytes(sh, 2, 148)
-    assert got >= 2 * rows * (w.d + 1) * 4 and got <= 2 * rows * (w.d + 1) * 4 + 1024
+    assert got >= 256 + 2 * rows * (w.d + 1) * 4 and got <= 256 + 2 * rows * (w.d + 1) * 4 + 1024
     # more splits than KV tiles are capped (no empty split, R10)
     tiles = -(-w.S_kv // 128)
     assert B.workspace_bytes(sh, 1000, 148) == B.workspace_bytes(sh, tiles, 148)
