@@ -116,6 +116,13 @@ __device__ __forceinline__ void umma_ss_lohi(uint32_t d_tmem, uint32_t a_lo, uin
         ::"r"(d_tmem), "r"(a_lo), "r"(b_lo), "r"(desc_hi), "r"(idesc), "r"(accumulate)
         : "memory");
 }
+// one 32-byte store (a whole sector) per lane; the address must be 32-byte aligned
+__device__ __forceinline__ void st_global_v8(void *ptr, uint32_t a, uint32_t b, uint32_t c, uint32_t d, uint32_t e, uint32_t f,
+                                             uint32_t g, uint32_t h) {
+    asm volatile("st.global.v8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"l"(ptr), "r"(a), "r"(b), "r"(c), "r"(d), "r"(e),
+                 "r"(f), "r"(g), "r"(h)
+                 : "memory");
+}
 // D[tmem] (+)= A[tmem] * B[smem]
 __device__ __forceinline__ void umma_ts_lohi(uint32_t d_tmem, uint32_t a_tmem, uint32_t b_lo, uint32_t desc_hi, uint32_t idesc,
                                              uint32_t accumulate) {
@@ -699,6 +706,7 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
                 const float lse = (m_tot + lg2_approx(l_tot)) * 0.6931471805599453f;
                 const float w_self = a_self * inv, w_other = a_other * inv;
                 const uint32_t tO_other = tmem + kOCol + 128u + lane_base;    // stream 1's accumulator, same rows
+                const bool o_align32 = (reinterpret_cast<uintptr_t>(p.O) & 31u) == 0;
                 if (p.n_splits == 1) {
                     if (row_ok) p.LSE[grow] = lse;
                 } else {
@@ -720,15 +728,17 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
                     }
                     if (row_ok) {
                         if (p.n_splits == 1) {
-                            uint4 *dst = reinterpret_cast<uint4 *>(p.O + grow * D + ch * 32);
+                            uint32_t u[16];
 #pragma unroll
-                            for (int q4 = 0; q4 < 4; ++q4) {
-                                uint4 u;
-                                u.x = pack_bf16x2(f[q4 * 8 + 0], f[q4 * 8 + 1]);
-                                u.y = pack_bf16x2(f[q4 * 8 + 2], f[q4 * 8 + 3]);
-                                u.z = pack_bf16x2(f[q4 * 8 + 4], f[q4 * 8 + 5]);
-                                u.w = pack_bf16x2(f[q4 * 8 + 6], f[q4 * 8 + 7]);
-                                dst[q4] = u;
+                            for (int e = 0; e < 16; ++e) u[e] = pack_bf16x2(f[2 * e], f[2 * e + 1]);
+                            uint16_t *dst = p.O + grow * D + ch * 32;
+                            if (o_align32) {              // whole 32-byte sectors per lane (rows are 2*D bytes apart)
+                                st_global_v8(dst, u[0], u[1], u[2], u[3], u[4], u[5], u[6], u[7]);
+                                st_global_v8(dst + 16, u[8], u[9], u[10], u[11], u[12], u[13], u[14], u[15]);
+                            } else {
+#pragma unroll
+                                for (int q4 = 0; q4 < 4; ++q4)
+                                    reinterpret_cast<uint4 *>(dst)[q4] = make_uint4(u[4 * q4], u[4 * q4 + 1], u[4 * q4 + 2], u[4 * q4 + 3]);
                             }
                         } else {
                             float4 *dst =
