@@ -17,6 +17,9 @@ __device__ __forceinline__ bool better(float v, int i, float bv, int bi) { retur
 __global__ void __launch_bounds__(kTopkWarps * 32) topk_kernel(const float *__restrict__ scores, int32_t *__restrict__ ids,
                                                                int rows, int N, int K) {
     extern __shared__ float smem_f[];
+    // let a dependent kernel (the attention, launched with programmatic stream serialization) become resident now;
+    // it waits for this grid's completion before it reads the ids
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int row = blockIdx.x * kTopkWarps + warp;
     if (row >= rows) return;
