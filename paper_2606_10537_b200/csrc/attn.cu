@@ -1,9 +1,10 @@
 // attn.cu -- a3 + a4 (+ the in-CTA half of a5): index-driven gather of the selected BOS+chunk KV rows and the
 // Split-S partial attention kernel (R7-R11), tcgen05 / TMEM, sm_100a.
 //
-// One persistent CTA per SM walks a list of work items.  An item belongs to one KV group (b, g) -- the G*L packed
-// query rows that share K/V (GQA groups sit in the MMA M dimension, so K/V are read once per group) -- and one split
-// of the virtual KV sequence [ K*Bk gathered cache rows || L_s decode-block rows ], cut at 128-row tile boundaries.
+// One persistent CTA per SM takes work items from an atomic counter (costliest first, so CTAs that finish early take
+// more).  An item belongs to one KV group (b, g) -- the G*L packed query rows that share K/V (GQA groups sit in the
+// MMA M dimension, so K/V are read once per group) -- and one split of the virtual KV sequence
+// [ K*Bk gathered cache rows || L_s decode-block rows ], cut at 128-row tile boundaries.
 // Every item runs TWO softmax streams that ping-pong on the tensor pipe (while one stream's 128 softmax threads
 // work on S, the tensor pipe runs the other stream's P*V and next Q*K^T):
 //   mode A (pair item)  : stream s owns query tile 2*pair+s; both streams walk the same KV tiles, so one K/V fetch
@@ -12,12 +13,14 @@
 //                         the CTA -- and the two (O, m, l) are merged by log-sum-exp in the epilogue, straight out of
 //                         TMEM (no HBM round trip).
 // Warp roles (416 threads): warps 0-3 softmax stream 0, warps 4-7 softmax stream 1 (thread = query row), warps 8-11
-// producers (16-byte cp.async row gather into 128B-swizzled panels; K and V of a tile share one index computation,
-// indices are prefetched a tile ahead so the gather runs at HBM speed), warp 12 issues every tcgen05.mma (one elected
-// lane, converged warp so the descriptors stay in uniform registers).
+// producers (16-byte cp.async row gather into 128B-swizzled panels; indices are prefetched a tile ahead so the gather
+// runs at HBM speed; completion is signalled by cp.async.mbarrier.arrive.noinc), warp 12 issues every tcgen05.mma
+// (one elected lane, converged warp so the descriptors stay in uniform registers).
 // TMEM (512 columns): S_s at 128*s (P aliases it as packed bf16), O_s at 256 + 128*s.
-// K/V ring: kStages tile slots; tile t of an item occupies loads 2*(t-t0) (K) and 2*(t-t0)+1 (V) counted from the
-// item's first load; a slot is released by a tcgen05.commit after its last user (stream 1 in mode A).
+// Shared memory: two Q tiles and a ring of kStages K/V tile slots; a single item needs one Q tile only and lends the
+// second Q buffer to the ring as a sixth slot (its two streams consume four tiles per step).  Ring state is a cursor
+// plus one phase bit per slot, kept alike by the producers and the MMA warp; a slot is released by a tcgen05.commit
+// after its last user (stream 1 in mode A).
 #include "pdllm_internal.h"
 #include "ptx.cuh"
 
