@@ -60,6 +60,9 @@ score_kernel(const ScoreParams p, const __grid_constant__ CUtensorMap tmap128, c
     __shared__ float s_ml[2][kTileM][2];      // column half 1's (m_ref, l) per row, double-buffered by chunk parity
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    // a dependent kernel (top-K, launched with programmatic stream serialization) may become resident beside this one;
+    // it waits for this grid's completion before it reads the scores
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     // persistent CTA: a contiguous range of the units u = ((bg * m_tiles + mt) * N + n)
     const int64_t u_lo = p.units * blockIdx.x / gridDim.x, u_hi = p.units * (blockIdx.x + 1) / gridDim.x;
     const int tiles_per_chunk = (p.Cp + kTileN - 1) / kTileN;

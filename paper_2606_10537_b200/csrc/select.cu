@@ -20,6 +20,8 @@ __global__ void __launch_bounds__(kTopkWarps * 32) topk_kernel(const float *__re
     // let a dependent kernel (the attention, launched with programmatic stream serialization) become resident now;
     // it waits for this grid's completion before it reads the ids
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    // ... and this kernel itself may have been launched under the kernel that writes the scores: wait for it
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int row = blockIdx.x * kTopkWarps + warp;
     if (row >= rows) return;
@@ -108,8 +110,19 @@ cudaError_t launch_topk(const Dims &s, const float *scores, int32_t *chunk_ids, 
         cudaError_t e = cudaFuncSetAttribute(topk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
     }
-    topk_kernel<<<(rows + kTopkWarps - 1) / kTopkWarps, kTopkWarps * 32, smem, st>>>(scores, chunk_ids, rows, s.N, s.K);
-    return cudaGetLastError();
+    // programmatic dependent launch: its blocks fit beside the score kernel's CTAs and start the moment it ends
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)((rows + kTopkWarps - 1) / kTopkWarps), 1, 1);
+    cfg.blockDim = dim3(kTopkWarps * 32, 1, 1);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    const int N = s.N, K = s.K;
+    return cudaLaunchKernelEx(&cfg, topk_kernel, scores, chunk_ids, rows, N, K);
 }
 
 cudaError_t launch_gather_idx(const Dims &s, const int32_t *chunk_ids, const int32_t *keep, int32_t *gather_idx,
