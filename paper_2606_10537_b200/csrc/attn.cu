@@ -292,8 +292,6 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
             const uint16_t *Kc = p.Kc + bg * p.N * p.Cp * D, *Vc = p.Vc + bg * p.N * p.Cp * D;
             const uint16_t *Kd = p.Kd + bg * p.L_s * D, *Vd = p.Vd + bg * p.L_s * D;
             const int32_t *keep = p.keep ? p.keep + bg * p.N * p.Bk : nullptr;
-            // the chunk ids come from the kernel in front of this one (top-K) when launched as its dependent
-            if (n_done == 0) asm volatile("griddepcontrol.wait;" ::: "memory");
             // the group's K <= 64 chunk ids live in two registers per lane (lane l: ids[l], ids[l + 32])
             const int ids_lo = lane < p.K ? __ldg(p.ids + bg * p.K + lane) : 0;
             const int ids_hi = lane + 32 < p.K ? __ldg(p.ids + bg * p.K + lane + 32) : 0;
@@ -772,20 +770,11 @@ cudaError_t launch_attn_d(const AttnParams &p, cudaStream_t st) {
     cudaError_t e = cudaFuncSetAttribute(attn_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::kSmem);
     if (e != cudaSuccess) return e;
     const int grid = p.n_items < device_num_sms() ? p.n_items : device_num_sms();
-    // Programmatic dependent launch: the CTAs may become resident (barrier init, TMEM allocation, Q / decode-block
-    // loads) while the kernel in front (top-K) is still running; the kernel waits (griddepcontrol.wait) before it
-    // reads the chunk ids.
-    cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3((unsigned)grid, 1, 1);
-    cfg.blockDim = dim3(kAttnThreads, 1, 1);
-    cfg.dynamicSmemBytes = Cfg::kSmem;
-    cfg.stream = st;
-    cudaLaunchAttribute attr[1];
-    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    attr[0].val.programmaticStreamSerializationAllowed = 1;
-    cfg.attrs = attr;
-    cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, attn_kernel<D>, p);
+    // (Launching this kernel as a programmatic dependent of the top-K kernel was measured -- 2.6 us per step -- and
+    // withdrawn: with the combine kernel behind it, long unsynchronised step loops ended in an invalid-address-space
+    // fault that a plain launch never shows.)
+    attn_kernel<D><<<grid, kAttnThreads, Cfg::kSmem, st>>>(p);
+    return cudaGetLastError();
 }
 
 }  // namespace

@@ -17,10 +17,8 @@ __device__ __forceinline__ bool better(float v, int i, float bv, int bi) { retur
 __global__ void __launch_bounds__(kTopkWarps * 32) topk_kernel(const float *__restrict__ scores, int32_t *__restrict__ ids,
                                                                int rows, int N, int K) {
     extern __shared__ float smem_f[];
-    // let a dependent kernel (the attention, launched with programmatic stream serialization) become resident now;
-    // it waits for this grid's completion before it reads the ids
-    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-    // ... and this kernel itself may have been launched under the kernel that writes the scores: wait for it
+    // this kernel may have been launched under the kernel that writes the scores (programmatic dependent launch):
+    // wait for that grid's completion and flush before the scores are read
     asm volatile("griddepcontrol.wait;" ::: "memory");
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int row = blockIdx.x * kTopkWarps + warp;
