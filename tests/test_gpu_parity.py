@@ -282,3 +282,29 @@ def test_scores_growing_logits(B):
 def test_attn_item_shapes(B, kw):
     w, inp = _inputs("tiny", **kw)
     _attn_case(B, w, inp, [0, 1, 3, 7])
+
+
+def test_step_back_to_back_without_sync(B):
+    """200 pdllm_step calls enqueued back to back (no host sync in between, the way a denoising loop runs them),
+    with and without the combine kernel: every call must reproduce the first, oracle-checked result bit for bit
+    (guards the launch-overlap plumbing: programmatic dependent launch, the work-item counter, workspace reuse)."""
+    w, inp = _inputs("tiny", C=300, H=8, H_kv=8, d=128, N=12, K=6, keep=1.0, L_q=64, L_d=192)
+    dev = to_device(inp)
+    shape = B.Shape.of(w)
+    ref = oracle.step(inp["Q_dec"], inp["Kcache"], inp["Vcache"], inp["keep"], inp["K_dec"], inp["V_dec"], w.K, w.L_q)
+    for S in (1, 2, 3):
+        ws = B.alloc_workspace(shape, S)
+        first = B.step(shape, dev["Q_dec"], dev["Kcache"], dev["Vcache"], dev["keep"], dev["K_dec"], dev["V_dec"],
+                       n_splits=S, workspace=ws)
+        torch.cuda.synchronize()
+        check_exact(first["chunk_ids"], ref["ids"])
+        check_O(first["O"], ref["O"], what=f"O (S={S})")
+        check_close(first["LSE"], ref["LSE"], LSE_ABS)
+        O0, L0 = first["O"].clone(), first["LSE"].clone()
+        out = dict(scores=first["scores"], chunk_ids=first["chunk_ids"], O=first["O"], LSE=first["LSE"])
+        for _ in range(200):
+            B.step(shape, dev["Q_dec"], dev["Kcache"], dev["Vcache"], dev["keep"], dev["K_dec"], dev["V_dec"],
+                   n_splits=S, workspace=ws, **out)
+        torch.cuda.synchronize()
+        assert torch.equal(out["O"].view(torch.int16), O0.view(torch.int16)), f"O changed across back-to-back steps (S={S})"
+        assert torch.equal(out["LSE"], L0), f"LSE changed across back-to-back steps (S={S})"
