@@ -29,11 +29,11 @@ cudaError_t launch_gather_idx(const Dims &s, const int32_t *chunk_ids, const int
 // ---- a5
 cudaError_t launch_combine(const float *O_part, const float *lse_part, int S, int64_t rows, int d, void *O, float *LSE,
                            cudaStream_t st);
-// ---- a1: scores[b,g,n]; `partial` is scratch of score_scratch_bytes()
-size_t score_scratch_bytes(const Dims &s);
+// ---- a1: scores[b,g,n]
 cudaError_t launch_score(const Dims &s, const void *Q, int64_t q_batch_stride, int64_t q_head_stride, const void *Kcache,
                          float *scores, cudaStream_t st);
-// ---- a3+a4 (+a5 when n_splits > 1)
+// ---- a3+a4 into O / LSE (n_splits == 1) or into the partials (n_splits > 1: launch_combine follows);
+// work_counter: one zeroed int32 (the persistent kernel's work-item counter)
 cudaError_t launch_attn(const Dims &s, const void *Q_dec, const void *Kcache, const void *Vcache, const int32_t *chunk_ids,
                         const int32_t *keep, const void *K_dec, const void *V_dec, int n_splits, void *O, float *LSE,
                         float *O_part, float *lse_part, int32_t *work_counter, cudaStream_t st);

@@ -2,12 +2,14 @@
 //
 //   scores[b,g,n] = mean over the G*L_q scoring rows of  log sum_{j<=C} exp(scale * q . Kcache[b,g,n,j])
 //
-// The kernel streams every cached K row exactly once (HBM-bound at MHA shapes).  One CTA owns a
-// 128-row tile of the scoring rows and a run of consecutive chunks of one (b,g); each chunk is
-// cut into 128-row K tiles (the tail tile is shortened to a multiple of 16 rows) that one thread
-// fetches with TMA into a ring of 128B-swizzled stages; one thread issues S = Q K^T (tcgen05.mma)
-// into one of two TMEM accumulators; the 128 softmax threads (thread = row) fold the tile into the
-// running (max, sum) of the current chunk and, at the chunk's last tile, reduce log-masses over rows.
+// The kernel streams every cached K row exactly once (HBM-bound at MHA shapes).  Persistent CTAs (two per SM) each take
+// an even share of the (b, g, M tile, chunk) units: a contiguous run of chunks, cut into segments of one (b, g, M tile)
+// whose 128-row tile of scoring rows is staged in shared memory.  Each chunk is cut into 128-row K tiles (the tail
+// tile is shortened to a multiple of 16 rows) that one thread fetches with TMA into a 2-stage ring of 128B-swizzled
+// panels; one thread issues S = Q K^T (tcgen05.mma) into one of two TMEM accumulators; 256 softmax threads (two per
+// row: columns 0-63 / 64-127 of every tile) fold the tile into their running (reference max, sum) of the current
+// chunk with one exp pass -- a quarter of the exponentials as an FMA-pipe polynomial, the tile's row sum as the overflow
+// detector -- and, at the chunk's last tile, merge the halves and reduce the log-masses over the rows.
 #include <cuda.h>
 
 #include "pdllm_internal.h"
