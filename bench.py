@@ -200,7 +200,9 @@ def workload_config(w, n_splits):
           if needs_flush(w) else
           "inputs larger than L2: the step streams the whole K cache "
           f"({w.score_bytes() / 1e6:.0f} MB) every iteration; no explicit flush")
-    return {"workload": f"BASELINE.json configs[{list(W.CONFIGS).index(w.name)}] '{w.name}'", "B": w.B, "H": w.H,
+    label = (f"BASELINE.json configs[{list(W.CONFIGS).index(w.name)}] '{w.name}'" if w.name in W.CONFIGS
+             else f"extra workload '{w.name}' (paper Fig. 5(b) decode shape; not a BASELINE.json config)")
+    return {"workload": label, "B": w.B, "H": w.H,
             "H_kv": w.H_kv, "d": w.d, "N": w.N, "C": w.C, "K": w.K, "keep": w.keep, "Bk": w.Bk, "L_q": w.L_q,
             "L_d": w.L_d, "prefix_tokens": w.N * w.C, "n_splits": n_splits,
             "call": "pdllm_step (score_chunks -> select_topk -> sparse_attn -> lse_combine)",
@@ -418,11 +420,11 @@ def main():
     ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=20)
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
-    ap.add_argument("--workload", choices=list(W.CONFIGS), default="sparse32k")
+    ap.add_argument("--workload", choices=list(W.CONFIGS) + list(W.EXTRA), default="sparse32k")
     ap.add_argument("--n-splits", type=int, default=0, help="0 = pdllm_auto_splits")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
-    w = W.CONFIGS[args.workload]
+    w = W.CONFIGS[args.workload] if args.workload in W.CONFIGS else W.EXTRA[args.workload]
     if args.impl == "reference":
         run_reference(args, w)
     else:

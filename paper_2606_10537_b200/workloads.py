@@ -79,6 +79,14 @@ CONFIGS = {
                           alpha=0.5, unit_logits=False, seed=BASE_SEED + 4),
 }
 
+# Not a BASELINE.json config: the paper's own decode-kernel shape (Fig. 5(b): GQA 32/8, d = 128, 32 rows per
+# head attending ~4K selected KV: K = 4 chunks of C = 1024), the L << S_kv regime Split-S was made for.
+# G*L = 128 packed rows = one query tile per KV group: 8 single items, so everything hangs on the split count.
+EXTRA = {
+    "fig5b": Workload("fig5b", B=1, H=32, H_kv=8, d=128, N=16, C=1024, K=4, keep=1.0, L_q=16, L_d=16,
+                      alpha=2.0, unit_logits=False, seed=BASE_SEED + 6),
+}
+
 
 def small_variant(w: Workload, **kw) -> Workload:
     return replace(w, **kw)

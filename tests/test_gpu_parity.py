@@ -308,3 +308,20 @@ def test_step_back_to_back_without_sync(B):
         torch.cuda.synchronize()
         assert torch.equal(out["O"].view(torch.int16), O0.view(torch.int16)), f"O changed across back-to-back steps (S={S})"
         assert torch.equal(out["LSE"], L0), f"LSE changed across back-to-back steps (S={S})"
+
+
+def test_step_fig5b_decode_shape(B):
+    """The paper's decode-kernel shape (Fig. 5(b)): GQA 32/8, 32 rows per head over ~4K selected KV -- one packed
+    query tile per KV group, so the whole call is Split-S (auto split count and the paper's S = 4)."""
+    w = W.EXTRA["fig5b"]
+    inp = W.make_inputs(w)
+    dev = to_device(inp)
+    shape = B.Shape.of(w)
+    ref = oracle.step(inp["Q_dec"], inp["Kcache"], inp["Vcache"], inp["keep"], inp["K_dec"], inp["V_dec"], w.K, w.L_q)
+    for S in (0, 4, 1):
+        out = B.step(shape, dev["Q_dec"], dev["Kcache"], dev["Vcache"], dev["keep"], dev["K_dec"], dev["V_dec"], n_splits=S)
+        torch.cuda.synchronize()
+        check_close(out["scores"], ref["scores"], SCORE_ABS, what="scores")
+        check_exact(out["chunk_ids"], ref["ids"])
+        check_O(out["O"], ref["O"], what=f"O (S={S})")
+        check_close(out["LSE"], ref["LSE"], LSE_ABS, what=f"LSE (S={S})")
