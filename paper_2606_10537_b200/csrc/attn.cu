@@ -25,13 +25,17 @@
 #include "ptx.cuh"
 
 #ifdef PDLLM_TRACE
-// Perf-debug build only (-DPDLLM_TRACE, never the shipped library): CTA 0 logs (clock64, code, arg) per role.
+// Perf-debug build only (-DPDLLM_TRACE, never the shipped library): one CTA logs (clock64, code, arg) per role.
 __device__ long long *g_pdllm_trace = nullptr;
+__device__ int g_pdllm_trace_cta = 0;
 extern "C" int pdllm_debug_set_trace(void *dev_buf) {
     return (int)cudaMemcpyToSymbol(g_pdllm_trace, &dev_buf, sizeof(void *));
 }
+extern "C" int pdllm_debug_set_trace_cta(int cta) {
+    return (int)cudaMemcpyToSymbol(g_pdllm_trace_cta, &cta, sizeof(int));
+}
 #define PDLLM_TRACE_DECL(role) \
-    longlong2 *tr_p = (blockIdx.x == 0 && g_pdllm_trace) ? reinterpret_cast<longlong2 *>(g_pdllm_trace) + (role) * 4096 : nullptr; \
+    longlong2 *tr_p = ((int)blockIdx.x == g_pdllm_trace_cta && g_pdllm_trace) ? reinterpret_cast<longlong2 *>(g_pdllm_trace) + (role) * 4096 : nullptr; \
     longlong2 *const tr_end = tr_p + 4096;
 #define PDLLM_TR(code, arg)                                                                       \
     do {                                                                                          \
@@ -183,7 +187,7 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
     __shared__ uint64_t bars[BAR_KV + 2 * (ST + 1)];
     __shared__ uint32_t tmem_slot;
     __shared__ int32_t s_items[4];                        // the CTA's next work items (ring, published by the producers)
-    __shared__ float s_ml[kSoftmaxThreads][2];            // mode B: stream 1's (m_ref, l) for the in-CTA merge
+    __shared__ float s_x[kTileM][2];                      // per-row exchange slots of the two column halves
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const uint32_t bar0 = smem_u32(&bars[0]);
@@ -197,9 +201,9 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
         mbar_init(bar(BAR_QFREE), 1);
         for (int s = 0; s < 2; ++s) {
             mbar_init(bar(BAR_SREADY0 + s), 1);
-            mbar_init(bar(BAR_PREADY0 + s), kSoftmaxThreads);
+            mbar_init(bar(BAR_PREADY0 + s), 2 * kSoftmaxThreads);
             mbar_init(bar(BAR_OREADY0 + s), 1);
-            mbar_init(bar(BAR_OFREE0 + s), kSoftmaxThreads);
+            mbar_init(bar(BAR_OFREE0 + s), 2 * kSoftmaxThreads);
         }
         for (int s = 0; s <= ST; ++s) {
             mbar_init(kv_full(s), kProducerThreads);
@@ -365,6 +369,7 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
             if (it.modeA) {
                 // tile by tile, K and V together (one index computation, one cp.async group): loads 2*jt and 2*jt + 1
                 prefetch_index(it.t0);
+                load_q();                                 // Q first: its rows need no indices, the first tile's are in flight
                 for (int jt = 0; jt < it.nt; ++jt) {
                     const int my_idx = nx_base + nx_raw;
                     if (pt == 0) PDLLM_TR(10, jt);
@@ -375,7 +380,6 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
                     if (pt == 0) PDLLM_TR(12, jt);
                     publish(kv_full(slot_k));
                     publish(kv_full(slot_v));
-                    if (jt == 0) load_q();
                 }
             } else {
                 // one tile per load, in the MMA warp's consumption order K(t0); { K(t0+i+1), V(t0+i) }; V(t0+nt-1)
@@ -390,15 +394,14 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
                     publish(kv_full(slot));
                 };
                 prefetch_index(it.t0);
+                load_q();
                 int idx_cur = nx_base + nx_raw;
                 if (it.nt > 1) prefetch_index(it.t0 + 1);
                 load_one(it.t0, idx_cur, false);
-                if (it.nt == 1) load_q();
                 for (int i = 0; i + 1 < it.nt; ++i) {
                     const int idx_new = nx_base + nx_raw;                       // tile t0 + i + 1
                     if (i + 2 < it.nt) prefetch_index(it.t0 + i + 2);
                     load_one(it.t0 + i + 1, idx_new, false);
-                    if (i == 0) load_q();                                       // Q goes in after the first two K tiles
                     load_one(it.t0 + i, idx_cur, true);
                     idx_cur = idx_new;
                 }
@@ -489,17 +492,20 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
                     if (lane == 0) PDLLM_TR(25, s);
                     const int ksteps = (int)(n_mma_of(tile) >> 4);
                     if (elect_one()) {
-                        // 16 kv rows per step: A = 8 TMEM columns of packed bf16 P, B = 16 V rows (MN-major, 2048 B)
+                        // 16 kv rows per step: A = 8 TMEM columns of packed bf16 P (column half h of the tile keeps its P at
+                        // S columns 64h..64h+31), B = 16 V rows (MN-major, 2048 B)
                         const int slot = v_slot;
                         const uint32_t v_lo = lo_v | ((sKV(slot) & 0x3FFFFu) >> 4);
                         const uint32_t tS = tmem + 128u * s, tO = tmem + kOCol + 128u * s;
                         if (ksteps == kTileN / 16) {
 #pragma unroll
                             for (int ks = 0; ks < kTileN / 16; ++ks)
-                                umma_ts_lohi(tO, tS + 8u * ks, v_lo + 128u * ks, hi_v, idesc_pv, (j > 0 || ks > 0) ? 1u : 0u);
+                                umma_ts_lohi(tO, tS + 64u * (ks >> 2) + 8u * (ks & 3), v_lo + 128u * ks, hi_v, idesc_pv,
+                                             (j > 0 || ks > 0) ? 1u : 0u);
                         } else {
                             for (int ks = 0; ks < ksteps; ++ks)
-                                umma_ts_lohi(tO, tS + 8u * ks, v_lo + 128u * ks, hi_v, idesc_pv, (j > 0 || ks > 0) ? 1u : 0u);
+                                umma_ts_lohi(tO, tS + 64u * (ks >> 2) + 8u * (ks & 3), v_lo + 128u * ks, hi_v, idesc_pv,
+                                             (j > 0 || ks > 0) ? 1u : 0u);
                         }
                         if (release) umma_commit(kv_free(slot));
                         if (last_pv) umma_commit(bar(BAR_OREADY0 + s));
@@ -512,214 +518,237 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
             }
         }
     } else {
-        // =============================== softmax streams (thread = query row) ===============================
-        const int s = warp >> 2;                          // stream
-        const int row = tid & (kSoftmaxThreads - 1);
+        // =============================== softmax (two threads per query row, both streams) ===============================
+        // A warp may only touch TMEM lanes 32*(warp%4)..+31 and warps w, w+4 sit on the same SM sub-partition, where a
+        // lone warp reaches only half the MUFU rate (measured: 590 clk per 32-column block alone, 352 clk each for two
+        // warps side by side).  So a query row is shared by two threads: half h = warp/4 owns columns 64h..64h+63 of
+        // every S tile (and columns D/2*h.. of the row's O accumulators), and the eight warps work through the tiles of
+        // BOTH streams in the order the MMA warp produces them: S(0,j), S(1,j), S(0,j+1), ...  Both halves use one
+        // reference max per row (P*V accumulates the whole row); their row sums are kept apart and added in the epilogue.
+        // P (packed bf16) goes over the first 32 of the thread's own 64 S columns, so the halves never touch each
+        // other's columns; they meet once per tile on a 64-thread named barrier that carries the overflow vote.
+        const int half = warp >> 2;
+        const int row = (warp & 3) * 32 + lane;
         const uint32_t lane_base = (uint32_t)((warp & 3) * 32) << 16;
-        const uint32_t tS = tmem + 128u * s + lane_base, tO = tmem + kOCol + 128u * s + lane_base;
-        uint32_t n_sready = 0, n_oready = 0;
-        int n_modeB = 0;
-        PDLLM_TRACE_DECL(2 + s)
+        constexpr int kOHalf = D / 2;                     // O columns per thread
+        const uint32_t pair_bar = 4u + (uint32_t)(warp & 3);
+        uint32_t ph_s = 0u, ph_o = 0u;                    // phase bits of S-ready / O-ready, bit s = stream s
+        PDLLM_TRACE_DECL(2 + half)
+        auto pair_sync = [&]() { asm volatile("bar.sync %0, 64;" ::"r"(pair_bar) : "memory"); };
+        auto pair_any = [&](bool pred) {
+            uint32_t r;
+            asm volatile(
+                "{\n\t.reg .pred p, q;\n\tsetp.ne.u32 p, %2, 0;\n\tbarrier.cta.red.or.pred.aligned q, %1, 64, p;\n\t"
+                "selp.u32 %0, 1, 0, q;\n\t}"
+                : "=r"(r)
+                : "r"(pair_bar), "r"((uint32_t)pred)
+                : "memory");
+            return r != 0;
+        };
+        // both halves' values of a per-row quantity (two pair barriers: publish, then release the slots)
+        auto pair_xch = [&](float v, float &v0, float &v1) {
+            s_x[row][half] = v;
+            pair_sync();
+            v0 = s_x[row][0];
+            v1 = s_x[row][1];
+            pair_sync();
+        };
+        if (row == 0) PDLLM_TR(1, 0);
         for (int n_done = 0;; ++n_done) {
             mbar_wait(bar(BAR_ITEM0 + (n_done & 3)), (uint32_t)(n_done >> 2) & 1u);
             const int ii = s_items[n_done & 3];
+            if (row == 0) PDLLM_TR(2, ii);
             if (ii < 0) break;
             const Item it = decode_item(p, ii);
-            const int n_mine = it.modeA ? it.nt : (s == 0 ? (it.nt + 1) / 2 : it.nt / 2);
-            float m_ref = -INFINITY, l = 0.f;
-            // multiply the O accumulator of this row by f (PV(s, j-1) completed before S(s, j) was committed)
-            auto scale_O = [&](float f) {
+            const int ns0 = it.modeA ? it.nt : (it.nt + 1) / 2, ns1 = it.modeA ? it.nt : it.nt / 2;    // tiles per stream
+            if (row == 0) PDLLM_TR(40, ii);
+            float m0 = -INFINITY, m1 = -INFINITY, l0 = 0.f, l1 = 0.f;     // per stream: reference max, this half's row sum
+            for (int j = 0; j < ns0; ++j) {
 #pragma unroll 1
-                for (int ch = 0; ch < D / 32; ++ch) {
-                    uint32_t o[32];
-                    tmem_ld32(tO + 32u * ch, o);
-                    tmem_wait_ld();
+                for (int s = 0; s < 2; ++s) {
+                    if (j >= (s ? ns1 : ns0)) continue;
+                    float m_ref = s ? m1 : m0, l = s ? l1 : l0;
+                    const uint32_t tSh = tmem + 128u * s + lane_base + 64u * half;      // this thread's 64 S columns
+                    const uint32_t tOh = tmem + kOCol + 128u * s + lane_base + (uint32_t)(kOHalf * half);
+                    const int tile = it.modeA ? it.t0 + j : it.t0 + 2 * j + s;
+                    const int n_valid = min(kTileN, p.S_kv - tile * kTileN);
+                    if (row == 0) PDLLM_TR(30, 2 * j + s);
+                    mbar_wait(bar(BAR_SREADY0 + s), (ph_s >> s) & 1u);
+                    ph_s ^= 1u << s;
+                    tc_fence_after();
+                    if (row == 0) PDLLM_TR(31, 2 * j + s);
+                    // one 32-column block of a full tile: P = 2^(c2*S - m_ref) as packed bf16 and its row sum; packed
+                    // f32x2 arithmetic (one FFMA2 / FADD2 per two columns), the exponentials on the MUFU pipe
+                    auto chunk_exp = [&](const uint32_t(&v)[32], uint32_t(&w)[16]) {
+                        const uint64_t c2v = pack_f32x2(p.c2, p.c2), mv = pack_f32x2(-m_ref, -m_ref);
+                        uint64_t acc0 = 0ull, acc1 = 0ull;
 #pragma unroll
-                    for (int e = 0; e < 32; ++e) o[e] = __float_as_uint(__uint_as_float(o[e]) * f);
-                    tmem_st32(tO + 32u * ch, o);
-                }
-            };
-            // one 32-column chunk of a FULL tile: P = 2^(c2*S - m_ref) as packed bf16 and its row sum; packed f32x2
-            // arithmetic (one FFMA2 / FADD2 per two columns), the exponentials on the MUFU pipe
-            auto chunk_exp = [&](const uint32_t(&v)[32], uint32_t(&w)[16]) {
-                const uint64_t c2v = pack_f32x2(p.c2, p.c2), mv = pack_f32x2(-m_ref, -m_ref);
-                uint64_t acc0 = 0ull, acc1 = 0ull;
-#pragma unroll
-                for (int e = 0; e < 32; e += 4) {
-                    float x0, x1, x2, x3;
-                    unpack_f32x2(fma_f32x2(pack_u32x2(v[e], v[e + 1]), c2v, mv), x0, x1);
-                    unpack_f32x2(fma_f32x2(pack_u32x2(v[e + 2], v[e + 3]), c2v, mv), x2, x3);
-                    const float p0 = ex2_approx(x0), p1 = ex2_approx(x1), p2 = ex2_approx(x2), p3 = ex2_approx(x3);
-                    acc0 = add_f32x2(acc0, pack_f32x2(p0, p1));
-                    acc1 = add_f32x2(acc1, pack_f32x2(p2, p3));
-                    w[e >> 1] = pack_bf16x2(p0, p1);
-                    w[(e >> 1) + 1] = pack_bf16x2(p2, p3);
-                }
-                float s0, s1, s2, s3;
-                unpack_f32x2(acc0, s0, s1);
-                unpack_f32x2(acc1, s2, s3);
-                return (s0 + s1) + (s2 + s3);
-            };
-            for (int j = 0; j < n_mine; ++j) {
-                const int tile = it.modeA ? it.t0 + j : it.t0 + 2 * j + s;
-                const int n_valid = min(kTileN, p.S_kv - tile * kTileN);
-                if (row == 0) PDLLM_TR(30, j);
-                mbar_wait(bar(BAR_SREADY0 + s), n_sready++ & 1u);
-                tc_fence_after();
-                if (row == 0) PDLLM_TR(31, j);
-                if (n_valid == kTileN) {
-                    if (j == 0) {
-                        // first tile of the stream: its row max becomes the reference (one extra pass over S)
-                        uint32_t v0[32], v1[32];
-                        float mx[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
-#pragma unroll 1
-                        for (int h = 0; h < 2; ++h) {
-                            tmem_ld32(tS + 64u * h, v0);
-                            tmem_ld32(tS + 64u * h + 32u, v1);
-                            tmem_wait_ld();
-#pragma unroll
-                            for (int e = 0; e < 32; ++e) mx[e & 3] = fmaxf(mx[e & 3], fmaxf(__uint_as_float(v0[e]), __uint_as_float(v1[e])));
-                        }
-                        m_ref = fmaxf(fmaxf(mx[0], mx[1]), fmaxf(mx[2], mx[3])) * p.c2;
-                    }
-                    // Single pass with the current reference max, TMEM loads one chunk ahead of the arithmetic.  The
-                    // chunk's row sum doubles as the overflow detector: some P > 2^13 implies sum > 2^13 (kSumLimit).
-                    // A chunk that trips it (rare) raises the reference by a whole number of octaves BEFORE its P is
-                    // stored: l, O and the P chunks already stored are rescaled by an exact power of two.
-                    float lsum = 0.f;
-                    uint32_t va[32], vb[32];
-                    auto do_chunk = [&](const uint32_t(&v)[32], int ch) {
-                        uint32_t w[16];
-                        float csum = chunk_exp(v, w);
-                        while (__any_sync(0xffffffffu, !(csum <= kSumLimit))) {
-                            float cmax = -INFINITY;
-#pragma unroll
-                            for (int e = 0; e < 32; ++e) cmax = fmaxf(cmax, __uint_as_float(v[e]));
-                            const float over = cmax * p.c2 - m_ref;
-                            const float up = !(csum <= kSumLimit) ? fmaxf(ceilf(over), 1.f) : 0.f;
-                            const float f = ex2_approx(-up);      // exact power of two (1 for rows that are fine)
-                            l *= f;
-                            lsum *= f;
-                            tmem_wait_st();
-                            rescale_tile(tS, tO, ch, D / 32, f);
-                            m_ref += up;
-                            csum = chunk_exp(v, w);
-                        }
-                        lsum += csum;
-                        tmem_st16(tS + 16u * ch, w);
-                        if (row == 0) PDLLM_TR(36, ch);
-                    };
-                    tmem_ld32(tS, va);
-                    tmem_wait_ld();
-#pragma unroll 1
-                    for (int h = 0; h < 2; ++h) {
-                        tmem_ld32(tS + 64u * h + 32u, vb);
-                        do_chunk(va, 2 * h);
-                        tmem_wait_ld();
-                        if (h == 0) tmem_ld32(tS + 64u, va);
-                        do_chunk(vb, 2 * h + 1);
-                        if (h == 0) tmem_wait_ld();
-                    }
-                    l += lsum;
-                } else {
-                    // first tile of the stream or a ragged tail tile: max pass, then exp pass with column masks
-                    const int n_mma = (n_valid + 15) & ~15;
-                    const int nchunks = (n_mma + 31) >> 5;
-                    float tmax = -INFINITY;
-                    for (int ch = 0; ch < nchunks; ++ch) {
-                        uint32_t v[32];
-                        tmem_ld32(tS + 32u * ch, v);
-                        tmem_wait_ld();
-                        float mx[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
-#pragma unroll
-                        for (int e = 0; e < 32; ++e)
-                            if (ch * 32 + e < n_valid) mx[e & 3] = fmaxf(mx[e & 3], __uint_as_float(v[e]));
-                        tmax = fmaxf(tmax, fmaxf(fmaxf(mx[0], mx[1]), fmaxf(mx[2], mx[3])));
-                    }
-                    const float tm2 = tmax * p.c2;
-                    const bool need = tm2 > m_ref + kRescaleThreshold;     // always true on the first tile
-                    if (__any_sync(0xffffffffu, need)) {
-                        const float m_new = need ? tm2 : m_ref;
-                        const float f = need ? ex2_approx(m_ref - m_new) : 1.f;   // m_ref = -inf -> 0
-                        l *= f;
-                        if (j > 0) scale_O(f);
-                        m_ref = m_new;
-                    }
-                    for (int ch = 0; ch < nchunks; ++ch) {
-                        uint32_t v[32];
-                        tmem_ld32(tS + 32u * ch, v);
-                        tmem_wait_ld();
-                        uint32_t w[16];
-                        float ls[4] = {0.f, 0.f, 0.f, 0.f};
-#pragma unroll
-                        for (int e = 0; e < 32; e += 2) {
-                            float p0 = ex2_approx(fmaf(__uint_as_float(v[e]), p.c2, -m_ref));
-                            float p1 = ex2_approx(fmaf(__uint_as_float(v[e + 1]), p.c2, -m_ref));
-                            if (ch * 32 + e >= n_valid) p0 = 0.f;
-                            if (ch * 32 + e + 1 >= n_valid) p1 = 0.f;
-                            ls[(e >> 1) & 3] += p0 + p1;
+                        for (int e = 0; e < 32; e += 4) {
+                            float x0, x1, x2, x3;
+                            unpack_f32x2(fma_f32x2(pack_u32x2(v[e], v[e + 1]), c2v, mv), x0, x1);
+                            unpack_f32x2(fma_f32x2(pack_u32x2(v[e + 2], v[e + 3]), c2v, mv), x2, x3);
+                            const float p0 = ex2_approx(x0), p1 = ex2_approx(x1), p2 = ex2_approx(x2), p3 = ex2_approx(x3);
+                            acc0 = add_f32x2(acc0, pack_f32x2(p0, p1));
+                            acc1 = add_f32x2(acc1, pack_f32x2(p2, p3));
                             w[e >> 1] = pack_bf16x2(p0, p1);
+                            w[(e >> 1) + 1] = pack_bf16x2(p2, p3);
                         }
-                        l += (ls[0] + ls[1]) + (ls[2] + ls[3]);
-                        tmem_st16(tS + 16u * ch, w);
+                        float s0, s1, s2, s3;
+                        unpack_f32x2(acc0, s0, s1);
+                        unpack_f32x2(acc1, s2, s3);
+                        return (s0 + s1) + (s2 + s3);
+                    };
+                    bool careful = !(n_valid == kTileN && j > 0);
+                    if (!careful) {
+                        // Single pass against the current reference.  The half-row sum doubles as the overflow detector
+                        // (some P > 2^14 implies sum > 2 * kSumLimit); an overflow anywhere in the two warps (rare) sends
+                        // the tile through the careful pass -- nothing has been stored yet, S is intact.
+                        uint32_t va[32], vb[32], w0[16], w1[16];
+                        tmem_ld32(tSh, va);
+                        tmem_wait_ld();
+                        if (row == 0) PDLLM_TR(36, 0);
+                        tmem_ld32(tSh + 32u, vb);
+                        float lsum = chunk_exp(va, w0);
+                        if (row == 0) PDLLM_TR(36, 1);
+                        tmem_wait_ld();
+                        lsum += chunk_exp(vb, w1);
+                        if (row == 0) PDLLM_TR(36, 2);
+                        careful = pair_any(!(lsum <= 2.f * kSumLimit));
+                        if (row == 0) PDLLM_TR(36, 3);
+                        if (!careful) {
+                            l += lsum;
+                            tmem_st16(tSh, w0);
+                            tmem_st16(tSh + 16u, w1);
+                        }
+                        if (row == 0) PDLLM_TR(36, 4);
+                    }
+                    if (careful) {
+                        // First tile of the stream, ragged tail tile, or after an overflow vote: row max over the valid
+                        // columns of both halves -> reference (raised by whole octaves once it exists, so that l and O
+                        // rescale exactly) -> masked exponentials -> P.  S is read twice.
+                        const int mine = max(0, min(64, n_valid - 64 * half));          // valid columns of this half
+                        float tmax = -INFINITY;
+#pragma unroll 1
+                        for (int b = 0; b < 2; ++b) {
+                            if (b * 32 >= mine) break;
+                            uint32_t v[32];
+                            tmem_ld32(tSh + 32u * b, v);
+                            tmem_wait_ld();
+                            float mx[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
+#pragma unroll
+                            for (int e = 0; e < 32; ++e)
+                                if (b * 32 + e < mine) mx[e & 3] = fmaxf(mx[e & 3], __uint_as_float(v[e]));
+                            tmax = fmaxf(tmax, fmaxf(fmaxf(mx[0], mx[1]), fmaxf(mx[2], mx[3])));
+                        }
+                        float t0, t1;
+                        pair_xch(tmax, t0, t1);
+                        const float tm2 = fmaxf(t0, t1) * p.c2;
+                        if (j == 0) {
+                            m_ref = tm2;                  // l = 0, O not started
+                        } else {
+                            const bool need = tm2 > m_ref + kRescaleThreshold;
+                            if (__any_sync(0xffffffffu, need)) {
+                                const float up = need ? ceilf(tm2 - m_ref) : 0.f;
+                                const float f = ex2_approx(-up);              // exact power of two (1 for rows that are fine)
+                                l *= f;
+                                // PV(s, j-1) completed before S(s, j) was committed: O is at rest
+#pragma unroll 1
+                                for (int ch = 0; ch < kOHalf / 32; ++ch) {
+                                    uint32_t o[32];
+                                    tmem_ld32(tOh + 32u * ch, o);
+                                    tmem_wait_ld();
+#pragma unroll
+                                    for (int e = 0; e < 32; ++e) o[e] = __float_as_uint(__uint_as_float(o[e]) * f);
+                                    tmem_st32(tOh + 32u * ch, o);
+                                }
+                                m_ref += up;
+                            }
+                        }
+                        uint32_t w[2][16];
+#pragma unroll
+                        for (int b = 0; b < 2; ++b) {
+#pragma unroll
+                            for (int e = 0; e < 16; ++e) w[b][e] = 0u;
+                            if (b * 32 < mine) {
+                                uint32_t v[32];
+                                tmem_ld32(tSh + 32u * b, v);
+                                tmem_wait_ld();
+                                float ls[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+                                for (int e = 0; e < 32; e += 2) {
+                                    float p0 = ex2_approx(fmaf(__uint_as_float(v[e]), p.c2, -m_ref));
+                                    float p1 = ex2_approx(fmaf(__uint_as_float(v[e + 1]), p.c2, -m_ref));
+                                    if (b * 32 + e >= mine) p0 = 0.f;
+                                    if (b * 32 + e + 1 >= mine) p1 = 0.f;
+                                    ls[(e >> 1) & 3] += p0 + p1;
+                                    w[b][e >> 1] = pack_bf16x2(p0, p1);
+                                }
+                                l += (ls[0] + ls[1]) + (ls[2] + ls[3]);
+                            }
+                        }
+                        tmem_st16(tSh, w[0]);
+                        tmem_st16(tSh + 16u, w[1]);
+                    }
+                    tmem_wait_st();
+                    tc_fence_before();
+                    mbar_arrive(bar(BAR_PREADY0 + s));
+                    if (row == 0) PDLLM_TR(33, 2 * j + s);
+                    if (s) {
+                        m1 = m_ref;
+                        l1 = l;
+                    } else {
+                        m0 = m_ref;
+                        l0 = l;
                     }
                 }
-                tmem_wait_st();
-                tc_fence_before();
-                mbar_arrive(bar(BAR_PREADY0 + s));
-                if (row == 0) PDLLM_TR(33, j);
             }
-            if (row == 0) PDLLM_TR(34, n_mine);
+            if (row == 0) PDLLM_TR(34, ns0);
             // ------------------------------- epilogue -------------------------------
-            const int qt = it.modeA ? it.q0 + s : it.q0;
-            const int qr = qt * kTileM + row;
-            const bool row_ok = qr < p.rows_g;
-            const int64_t grow = (int64_t)it.bg * p.rows_g + qr;
-            if (n_mine > 0) {
-                mbar_wait(bar(BAR_OREADY0 + s), n_oready++ & 1u);
-                tc_fence_after();
-            }
-            float a_self = 1.f, a_other = 0.f, l_tot = l, m_tot = m_ref;
-            const bool merge_other = !it.modeA && it.nt > 1;    // stream 1 had tiles (uniform per item)
-            if (!it.modeA) {
-                // a5 inside the CTA: stream 1 publishes (m, l); stream 0 merges both accumulators out of TMEM
-                if (s == 1) {
-                    // stream 0 has read the previous single item's pair (named barrier 3: it arrives, we wait)
-                    if (n_modeB > 0) asm volatile("bar.sync 3, 256;" ::: "memory");
-                    s_ml[row][0] = m_ref;
-                    s_ml[row][1] = l;
+            // Pair items: one output tile per stream.  Single items (a5 inside the CTA): both streams hold partial
+            // results of the SAME rows, merged here out of TMEM -- every thread already has both (m, l) pairs.
+            const bool merge_other = !it.modeA && it.nt > 1;      // stream 1 had tiles (uniform per item)
+            const bool o_align32 = (reinterpret_cast<uintptr_t>(p.O) & 31u) == 0;
+            const int n_out = it.modeA ? 2 : 1;
+#pragma unroll 1
+            for (int s = 0; s < n_out; ++s) {
+                const int qr = (it.q0 + s) * kTileM + row;
+                const bool row_ok = qr < p.rows_g;
+                const int64_t grow = (int64_t)it.bg * p.rows_g + qr;
+                mbar_wait(bar(BAR_OREADY0 + s), (ph_o >> s) & 1u);
+                ph_o ^= 1u << s;
+                if (merge_other) {
+                    mbar_wait(bar(BAR_OREADY1), (ph_o >> 1) & 1u);
+                    ph_o ^= 2u;
                 }
-                ++n_modeB;
-                tc_fence_before();
-                asm volatile("bar.sync 2, 256;" ::: "memory");
                 tc_fence_after();
-                if (s == 0) {
-                    const float m1 = s_ml[row][0], l1 = s_ml[row][1];
-                    asm volatile("bar.arrive 3, 256;" ::: "memory");
-                    if (merge_other) {
-                        m_tot = fmaxf(m_ref, m1);
-                        a_self = ex2_approx(m_ref - m_tot);
-                        a_other = ex2_approx(m1 - m_tot);
-                        l_tot = l * a_self + l1 * a_other;
-                    }
+                if (row == 0) PDLLM_TR(37, s);
+                float x0, x1;
+                pair_xch(s ? l1 : l0, x0, x1);
+                if (row == 0) PDLLM_TR(38, s);
+                const float l_row = x0 + x1;
+                float a_self = 1.f, a_other = 0.f, l_tot = l_row, m_tot = s ? m1 : m0;
+                if (merge_other) {
+                    pair_xch(l1, x0, x1);
+                    m_tot = fmaxf(m0, m1);
+                    a_self = ex2_approx(m0 - m_tot);
+                    a_other = ex2_approx(m1 - m_tot);
+                    l_tot = l_row * a_self + (x0 + x1) * a_other;
                 }
-            }
-            if (it.modeA || s == 0) {
                 const float inv = 1.f / l_tot;
                 const float lse = (m_tot + lg2_approx(l_tot)) * 0.6931471805599453f;
                 const float w_self = a_self * inv, w_other = a_other * inv;
-                const uint32_t tO_other = tmem + kOCol + 128u + lane_base;    // stream 1's accumulator, same rows
-                const bool o_align32 = (reinterpret_cast<uintptr_t>(p.O) & 31u) == 0;
-                if (p.n_splits == 1) {
-                    if (row_ok) p.LSE[grow] = lse;
-                } else {
-                    if (row_ok) p.lse_part[(int64_t)it.split * p.total_rows + grow] = lse;
+                const uint32_t tOh = tmem + kOCol + 128u * s + lane_base + (uint32_t)(kOHalf * half);
+                const uint32_t tO_other = tmem + kOCol + 128u + lane_base + (uint32_t)(kOHalf * half);    // stream 1, same rows
+                if (half == 0 && row_ok) {
+                    if (p.n_splits == 1) p.LSE[grow] = lse;
+                    else p.lse_part[(int64_t)it.split * p.total_rows + grow] = lse;
                 }
 #pragma unroll 1
-                for (int ch = 0; ch < D / 32; ++ch) {
+                for (int ch = 0; ch < kOHalf / 32; ++ch) {
                     uint32_t o[32];
-                    tmem_ld32(tO + 32u * ch, o);
+                    tmem_ld32(tOh + 32u * ch, o);
                     tmem_wait_ld();
+                    if (row == 0) PDLLM_TR(41, ch);
                     float f[32];
 #pragma unroll
                     for (int e = 0; e < 32; ++e) f[e] = __uint_as_float(o[e]) * w_self;
@@ -730,11 +759,12 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
                         for (int e = 0; e < 32; ++e) f[e] = fmaf(__uint_as_float(o[e]), w_other, f[e]);
                     }
                     if (row_ok) {
+                        const int col0 = kOHalf * half + ch * 32;
                         if (p.n_splits == 1) {
                             uint32_t u[16];
 #pragma unroll
                             for (int e = 0; e < 16; ++e) u[e] = pack_bf16x2(f[2 * e], f[2 * e + 1]);
-                            uint16_t *dst = p.O + grow * D + ch * 32;
+                            uint16_t *dst = p.O + grow * D + col0;
                             if (o_align32) {              // whole 32-byte sectors per lane (rows are 2*D bytes apart)
                                 st_global_v8(dst, u[0], u[1], u[2], u[3], u[4], u[5], u[6], u[7]);
                                 st_global_v8(dst + 16, u[8], u[9], u[10], u[11], u[12], u[13], u[14], u[15]);
@@ -745,18 +775,20 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
                             }
                         } else {
                             float4 *dst =
-                                reinterpret_cast<float4 *>(p.O_part + ((int64_t)it.split * p.total_rows + grow) * D + ch * 32);
+                                reinterpret_cast<float4 *>(p.O_part + ((int64_t)it.split * p.total_rows + grow) * D + col0);
 #pragma unroll
                             for (int q4 = 0; q4 < 8; ++q4)
                                 dst[q4] = make_float4(f[q4 * 4 + 0], f[q4 * 4 + 1], f[q4 * 4 + 2], f[q4 * 4 + 3]);
                         }
                     }
+                    if (row == 0) PDLLM_TR(42, ch);
                 }
+                if (row == 0) PDLLM_TR(39, s);
                 tc_fence_before();
                 mbar_arrive(bar(BAR_OFREE0 + s));
-                if (merge_other) mbar_arrive(bar(BAR_OFREE1));      // stream 0 has drained stream 1's accumulator
+                if (merge_other) mbar_arrive(bar(BAR_OFREE1));      // stream 1's accumulator has been drained too
             }
-            if (row == 0) PDLLM_TR(35, n_mine);
+            if (row == 0) PDLLM_TR(35, ns0);
         }
     }
     tc_fence_before();
