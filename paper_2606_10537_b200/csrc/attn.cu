@@ -481,9 +481,12 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
                     // the loads this stream step needs have normally landed long ago: cross them into the async proxy
                     // BEFORE waiting for P, so that P*V and the next Q*K^T issue back to back once P is there
                     if (fresh) {
+                        if (lane == 0) PDLLM_TR(27, j);
                         v_slot = next_load();
                         if (has_next) k_slot = next_load();
+                        if (lane == 0) PDLLM_TR(28, j);
                         fence_proxy_async_smem();
+                        if (lane == 0) PDLLM_TR(29, j);
                     }
                     if (lane == 0) PDLLM_TR(23, s);
                     mbar_wait(bar(BAR_PREADY0 + s), n_pready[s]++ & 1u);
@@ -598,7 +601,20 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
                         unpack_f32x2(acc1, s2, s3);
                         return (s0 + s1) + (s2 + s3);
                     };
-                    bool careful = !(n_valid == kTileN && j > 0);
+                    bool careful = n_valid != kTileN;
+                    if (!careful && j == 0) {
+                        // first tile of the stream (full): its row max becomes the reference (one extra pass over S)
+                        uint32_t va[32], vb[32];
+                        tmem_ld32(tSh, va);
+                        tmem_ld32(tSh + 32u, vb);
+                        tmem_wait_ld();
+                        float mx[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
+#pragma unroll
+                        for (int e = 0; e < 32; ++e) mx[e & 3] = fmaxf(mx[e & 3], fmaxf(__uint_as_float(va[e]), __uint_as_float(vb[e])));
+                        float t0, t1;
+                        pair_xch(fmaxf(fmaxf(mx[0], mx[1]), fmaxf(mx[2], mx[3])), t0, t1);
+                        m_ref = fmaxf(t0, t1) * p.c2;
+                    }
                     if (!careful) {
                         // Single pass against the current reference.  The half-row sum doubles as the overflow detector
                         // (some P > 2^14 implies sum > 2 * kSumLimit); an overflow anywhere in the two warps (rare) sends
@@ -623,7 +639,7 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
                         if (row == 0) PDLLM_TR(36, 4);
                     }
                     if (careful) {
-                        // First tile of the stream, ragged tail tile, or after an overflow vote: row max over the valid
+                        // Ragged tail tile (possibly the stream's first) or after an overflow vote: row max over the valid
                         // columns of both halves -> reference (raised by whole octaves once it exists, so that l and O
                         // rescale exactly) -> masked exponentials -> P.  S is read twice.
                         const int mine = max(0, min(64, n_valid - 64 * half));          // valid columns of this half
@@ -709,30 +725,28 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
             const bool merge_other = !it.modeA && it.nt > 1;      // stream 1 had tiles (uniform per item)
             const bool o_align32 = (reinterpret_cast<uintptr_t>(p.O) & 31u) == 0;
             const int n_out = it.modeA ? 2 : 1;
+            // whole-row sums (both halves), exchanged while the last P*V are still running
+            float lr0, lr1 = 0.f;
+            {
+                float x0, x1;
+                pair_xch(l0, x0, x1);
+                lr0 = x0 + x1;
+                if (it.modeA || merge_other) {
+                    pair_xch(l1, x0, x1);
+                    lr1 = x0 + x1;
+                }
+            }
 #pragma unroll 1
             for (int s = 0; s < n_out; ++s) {
                 const int qr = (it.q0 + s) * kTileM + row;
                 const bool row_ok = qr < p.rows_g;
                 const int64_t grow = (int64_t)it.bg * p.rows_g + qr;
-                mbar_wait(bar(BAR_OREADY0 + s), (ph_o >> s) & 1u);
-                ph_o ^= 1u << s;
+                float a_self = 1.f, a_other = 0.f, l_tot = s ? lr1 : lr0, m_tot = s ? m1 : m0;
                 if (merge_other) {
-                    mbar_wait(bar(BAR_OREADY1), (ph_o >> 1) & 1u);
-                    ph_o ^= 2u;
-                }
-                tc_fence_after();
-                if (row == 0) PDLLM_TR(37, s);
-                float x0, x1;
-                pair_xch(s ? l1 : l0, x0, x1);
-                if (row == 0) PDLLM_TR(38, s);
-                const float l_row = x0 + x1;
-                float a_self = 1.f, a_other = 0.f, l_tot = l_row, m_tot = s ? m1 : m0;
-                if (merge_other) {
-                    pair_xch(l1, x0, x1);
                     m_tot = fmaxf(m0, m1);
                     a_self = ex2_approx(m0 - m_tot);
                     a_other = ex2_approx(m1 - m_tot);
-                    l_tot = l_row * a_self + (x0 + x1) * a_other;
+                    l_tot = lr0 * a_self + lr1 * a_other;
                 }
                 const float inv = 1.f / l_tot;
                 const float lse = (m_tot + lg2_approx(l_tot)) * 0.6931471805599453f;
@@ -743,12 +757,21 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
                     if (p.n_splits == 1) p.LSE[grow] = lse;
                     else p.lse_part[(int64_t)it.split * p.total_rows + grow] = lse;
                 }
-#pragma unroll 1
-                for (int ch = 0; ch < kOHalf / 32; ++ch) {
-                    uint32_t o[32];
-                    tmem_ld32(tOh + 32u * ch, o);
-                    tmem_wait_ld();
-                    if (row == 0) PDLLM_TR(41, ch);
+                mbar_wait(bar(BAR_OREADY0 + s), (ph_o >> s) & 1u);
+                ph_o ^= 1u << s;
+                if (merge_other) {
+                    mbar_wait(bar(BAR_OREADY1), (ph_o >> 1) & 1u);
+                    ph_o ^= 2u;
+                }
+                tc_fence_after();
+                if (row == 0) PDLLM_TR(37, s);
+                constexpr int kCh = kOHalf / 32;          // 32-column chunks of this thread's O columns (1 or 2)
+                uint32_t oa[32], ob[32];
+                tmem_ld32(tOh, oa);
+                if (kCh == 2) tmem_ld32(tOh + 32u, ob);
+                tmem_wait_ld();
+                if (row == 0) PDLLM_TR(38, s);
+                auto emit = [&](uint32_t(&o)[32], int ch) {
                     float f[32];
 #pragma unroll
                     for (int e = 0; e < 32; ++e) f[e] = __uint_as_float(o[e]) * w_self;
@@ -781,12 +804,22 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
                                 dst[q4] = make_float4(f[q4 * 4 + 0], f[q4 * 4 + 1], f[q4 * 4 + 2], f[q4 * 4 + 3]);
                         }
                     }
-                    if (row == 0) PDLLM_TR(42, ch);
+                };
+                if (merge_other) {
+                    // stream 1's chunk comes through the same registers: one chunk at a time
+                    emit(oa, 0);
+                    if (kCh == 2) emit(ob, 1);
+                    tc_fence_before();
+                    mbar_arrive(bar(BAR_OFREE0));
+                    mbar_arrive(bar(BAR_OFREE1));         // stream 1's accumulator has been drained too
+                } else {
+                    // the accumulator is in registers: hand it back before the stores
+                    tc_fence_before();
+                    mbar_arrive(bar(BAR_OFREE0 + s));
+                    emit(oa, 0);
+                    if (kCh == 2) emit(ob, 1);
                 }
                 if (row == 0) PDLLM_TR(39, s);
-                tc_fence_before();
-                mbar_arrive(bar(BAR_OFREE0 + s));
-                if (merge_other) mbar_arrive(bar(BAR_OFREE1));      // stream 1's accumulator has been drained too
             }
             if (row == 0) PDLLM_TR(35, ns0);
         }
