@@ -284,7 +284,8 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
         // finish early take more; thread 0 of the producers fetches, the other roles follow through s_items.
         for (;; ++n_done) {
             if (pt == 0) {
-                const int nxt = atomicAdd(p.work_counter, 1);
+                // the first item of a CTA is its block index (no round trip to the counter at kernel start)
+                const int nxt = n_done == 0 ? (int)blockIdx.x : (int)gridDim.x + atomicAdd(p.work_counter, 1);
                 s_items[n_done & 3] = nxt < p.n_items ? nxt : -1;
             }
             asm volatile("bar.sync 1, 128;" ::: "memory");
