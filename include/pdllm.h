@@ -185,10 +185,16 @@ int pdllm_step_profiled(const pdllm_shape *shape, const void *Q_dec, const void 
  * The prefix cache and keep lists are state that the prefill left on the device
  * ("static cache that is reused across all T denoising steps"); what
  * changes every step is the decode block.  This call enqueues, on `stream`:
- * H2D copies of h_Q_dec/h_K_dec/h_V_dec (host, pinned for true async) into
- * d_scratch, pdllm_step, and D2H copies of O, LSE and chunk ids into the host
- * outputs.  The caller synchronises the stream before reading them.
- *   d_scratch  device scratch of >= pdllm_step_host_scratch_bytes() bytes         */
+ * the H2D copy of h_Q_dec (host, pinned for true async) into d_scratch, the
+ * steps of pdllm_step, and D2H copies of O, LSE and chunk ids into the host
+ * outputs.  h_K_dec / h_V_dec, which only the attention reads, are copied on a
+ * side stream the library owns (one per host thread and device, created on
+ * first use): it forks from `stream` at the start of the call and joins it
+ * ahead of the attention kernel, so those copies run under the scoring kernel;
+ * to the caller all work is ordered on `stream`, which it synchronises before
+ * reading the outputs.
+ *   d_scratch  device scratch of >= pdllm_step_host_scratch_bytes() bytes; one
+ *              call at a time may use it                                          */
 int pdllm_step_host(const pdllm_shape *shape, const void *h_Q_dec, const void *h_K_dec,
                     const void *h_V_dec, const void *d_Kcache, const void *d_Vcache,
                     const int32_t *d_token_keep_idx, int32_t n_splits,

@@ -238,6 +238,26 @@ int attn_impl(const Dims &d, const void *Q_dec, const void *Kcache, const void *
     return record(ev_end, st);
 }
 
+// The side stream of pdllm_step_host (one per host thread and device, created on first use, kept for the process).
+struct SideStream {
+    cudaStream_t stream = nullptr;
+    cudaEvent_t fork = nullptr, join = nullptr;
+    int device = -1;
+};
+SideStream *side_stream() {
+    static thread_local SideStream ss[16];
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 16) return nullptr;
+    SideStream &s = ss[dev];
+    if (s.device != dev) {
+        if (cudaStreamCreateWithFlags(&s.stream, cudaStreamNonBlocking) != cudaSuccess) return nullptr;
+        if (cudaEventCreateWithFlags(&s.fork, cudaEventDisableTiming) != cudaSuccess) return nullptr;
+        if (cudaEventCreateWithFlags(&s.join, cudaEventDisableTiming) != cudaSuccess) return nullptr;
+        s.device = dev;
+    }
+    return &s;
+}
+
 int attn_validate(const pdllm_shape *shape, const void *Q_dec, const void *Kcache, const void *Vcache,
                   const int32_t *chunk_ids, const int32_t *token_keep_idx, const void *K_dec, const void *V_dec,
                   int32_t n_splits, void *O, float *LSE, void *workspace, size_t workspace_bytes, Dims *d, int *S) {
@@ -318,13 +338,34 @@ int pdllm_step_host(const pdllm_shape *shape, const void *h_Q_dec, const void *h
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     char *base = static_cast<char *>(d_scratch);
     const size_t qb = (size_t)d.B * d.H * d.L * d.d * 2, kb = (size_t)d.B * d.H_kv * d.L_s * d.d * 2;
+    int32_t *ids = reinterpret_cast<int32_t *>(base + h.ids);
+    float *scores = reinterpret_cast<float *>(base + h.scores);
+    Dims dv;
+    int Sv = 1;
+    if (int rc = attn_validate(shape, base + h.q, d_Kcache, d_Vcache, ids, d_token_keep_idx, base + h.kd, base + h.vd,
+                               n_splits, base + h.o, reinterpret_cast<float *>(base + h.lse), base + h.ws, h.total - h.ws,
+                               &dv, &Sv))
+        return rc;
+    if (shape->L_q > shape->L) return PDLLM_ERR_SHAPE;
+    // Scoring and top-K need only Q: K_dec / V_dec travel on a library-owned side stream underneath them and join
+    // before the attention (fork after everything queued on `stream`, so an earlier step's kernels have let go of
+    // the scratch buffers).
+    SideStream *ss = side_stream();
+    if (!ss) return PDLLM_ERR_CUDA;
+    if (cudaEventRecord(ss->fork, st) != cudaSuccess) return PDLLM_ERR_CUDA;
+    if (cudaStreamWaitEvent(ss->stream, ss->fork, 0) != cudaSuccess) return PDLLM_ERR_CUDA;
     if (cudaMemcpyAsync(base + h.q, h_Q_dec, qb, cudaMemcpyHostToDevice, st) != cudaSuccess) return PDLLM_ERR_CUDA;
-    if (cudaMemcpyAsync(base + h.kd, h_K_dec, kb, cudaMemcpyHostToDevice, st) != cudaSuccess) return PDLLM_ERR_CUDA;
-    if (cudaMemcpyAsync(base + h.vd, h_V_dec, kb, cudaMemcpyHostToDevice, st) != cudaSuccess) return PDLLM_ERR_CUDA;
-    if (int rc = pdllm_step(shape, base + h.q, d_Kcache, d_Vcache, d_token_keep_idx, base + h.kd, base + h.vd, n_splits,
-                            reinterpret_cast<float *>(base + h.scores), reinterpret_cast<int32_t *>(base + h.ids),
-                            base + h.o, reinterpret_cast<float *>(base + h.lse), nullptr, base + h.ws,
-                            h.total - h.ws, stream))
+    if (cudaMemcpyAsync(base + h.kd, h_K_dec, kb, cudaMemcpyHostToDevice, ss->stream) != cudaSuccess) return PDLLM_ERR_CUDA;
+    if (cudaMemcpyAsync(base + h.vd, h_V_dec, kb, cudaMemcpyHostToDevice, ss->stream) != cudaSuccess) return PDLLM_ERR_CUDA;
+    if (cudaEventRecord(ss->join, ss->stream) != cudaSuccess) return PDLLM_ERR_CUDA;
+    if (int rc = cuda_rc(cudaMemsetAsync(base + h.ws, 0, sizeof(int32_t), st))) return rc;
+    if (int rc = cuda_rc(launch_score(dv, base + h.q, (int64_t)dv.H * dv.L * dv.d, (int64_t)dv.L * dv.d, d_Kcache, scores, st)))
+        return rc;
+    if (int rc = cuda_rc(launch_topk(dv, scores, ids, st))) return rc;
+    if (cudaStreamWaitEvent(st, ss->join, 0) != cudaSuccess) return PDLLM_ERR_CUDA;
+    if (int rc = attn_impl(dv, base + h.q, d_Kcache, d_Vcache, ids, d_token_keep_idx, base + h.kd, base + h.vd, Sv,
+                           base + h.o, reinterpret_cast<float *>(base + h.lse), nullptr, base + h.ws, true, nullptr, nullptr,
+                           st))
         return rc;
     if (cudaMemcpyAsync(h_O, base + h.o, qb, cudaMemcpyDeviceToHost, st) != cudaSuccess) return PDLLM_ERR_CUDA;
     if (cudaMemcpyAsync(h_LSE, base + h.lse, (size_t)d.B * d.H * d.L * 4, cudaMemcpyDeviceToHost, st) != cudaSuccess)
