@@ -325,3 +325,32 @@ def test_step_fig5b_decode_shape(B):
         check_exact(out["chunk_ids"], ref["ids"])
         check_O(out["O"], ref["O"], what=f"O (S={S})")
         check_close(out["LSE"], ref["LSE"], LSE_ABS, what=f"LSE (S={S})")
+
+
+@pytest.mark.parametrize("half", [0, 1])
+@pytest.mark.parametrize("d", [64, 128])
+def test_attn_overflow_in_one_column_half(B, half, d):
+    """A query row is shared by two softmax threads (columns 0..63 and 64..127 of every 128-key tile).  Here the
+    logits outgrow the reference max, tile after tile, ONLY in the columns of one half: the other half sees nothing
+    unusual and has to follow the pair's overflow vote (same reference, same rescale) for the row to come out right."""
+    w, inp = _inputs("tiny", C=255, K=4, N=4, keep=1.0, L_q=96, L_d=160, H=4, H_kv=2, d=d)      # K = N: virtual row = cache row
+    u = np.zeros(w.d, np.float32); u[::2] = 1.0; u /= np.linalg.norm(u)
+    Q = W.bf16_bits_to_f32(inp["Q_dec"]) + 4.0 * u
+    Kc = W.bf16_bits_to_f32(inp["Kcache"]).copy()                  # [B, H_kv, N, Cp, d]
+    v = np.arange(w.N * w.Cp).reshape(w.N, w.Cp)                   # position in the gathered sequence
+    boost = np.where((v % 128) // 64 == half, 12.0 * (v // 128), 0.0).astype(np.float32)        # +12*sqrt(d)/8.. per tile
+    Kc += (boost[..., None] * u * (np.sqrt(w.d) / 4.0))[None, None]
+    inp["Q_dec"], inp["Kcache"] = W.f32_to_bf16_bits(Q), W.f32_to_bf16_bits(Kc)
+    _attn_case(B, w, inp, [1, 2])
+
+
+@pytest.mark.parametrize("tail", [1, 33, 64, 65, 97, 127])
+def test_attn_ragged_tail_widths(B, tail):
+    """Last KV tile with `tail` valid keys: 1..64 leaves the second column half of the tile empty, 65..127 masks inside
+    it; pair items and a single item (L = 300: three query tiles), with and without splits."""
+    L = 300
+    S_pre = 2 * 101                                                # K = 2 chunks of C + 1 = 101 kept whole
+    L_s = next(x for x in range(L, L + 128) if (S_pre + x) % 128 == tail)
+    w, inp = _inputs("tiny", C=100, K=2, keep=1.0, L_q=40, L_d=L_s - 40, H=2, H_kv=2, d=128)
+    assert (w.K * (w.C + 1) + w.L) % 128 == tail
+    _attn_case(B, w, inp, [1, 2])
