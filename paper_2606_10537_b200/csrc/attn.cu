@@ -5,18 +5,19 @@
 // more).  An item belongs to one KV group (b, g) -- the G*L packed query rows that share K/V (GQA groups sit in the
 // MMA M dimension, so K/V are read once per group) -- and one split of the virtual KV sequence
 // [ K*Bk gathered cache rows || L_s decode-block rows ], cut at 128-row tile boundaries.
-// Every item runs TWO softmax streams that ping-pong on the tensor pipe (while one stream's 128 softmax threads
-// work on S, the tensor pipe runs the other stream's P*V and next Q*K^T):
+// Every item runs TWO streams -- two (S/P, O) accumulator sets in TMEM whose MMAs alternate on the tensor pipe (while
+// the softmax warps work on one stream's S, the tensor pipe runs the other stream's P*V and next Q*K^T):
 //   mode A (pair item)  : stream s owns query tile 2*pair+s; both streams walk the same KV tiles, so one K/V fetch
 //                         feeds 256 query rows (halves the L2->SM traffic of 128-row CTAs);
 //   mode B (single item): the group's odd last query tile; stream s walks KV tiles t0+s, t0+s+2, ... -- Split-S inside
 //                         the CTA -- and the two (O, m, l) are merged by log-sum-exp in the epilogue, straight out of
 //                         TMEM (no HBM round trip).
-// Warp roles (416 threads): warps 0-3 softmax stream 0, warps 4-7 softmax stream 1 (thread = query row), warps 8-11
+// Warp roles (416 threads): warps 0-7 softmax, two threads per query row (warps 0-3 columns 0-63, warps 4-7 columns
+// 64-127 of every S tile), working through the tiles of both streams in the order they are produced; warps 8-11
 // producers (16-byte cp.async row gather into 128B-swizzled panels; indices are prefetched a tile ahead so the gather
 // runs at HBM speed; completion is signalled by cp.async.mbarrier.arrive.noinc), warp 12 issues every tcgen05.mma
 // (one elected lane, converged warp so the descriptors stay in uniform registers).
-// TMEM (512 columns): S_s at 128*s (P aliases it as packed bf16), O_s at 256 + 128*s.
+// TMEM (512 columns): S_s at 128*s (P aliases it as packed bf16: column half h at 128*s + 64*h .. + 31), O_s at 256 + 128*s.
 // Shared memory: two Q tiles and a ring of kStages K/V tile slots; a single item needs one Q tile only and lends the
 // second Q buffer to the ring as a sixth slot (its two streams consume four tiles per step).  Ring state is a cursor
 // plus one phase bit per slot, kept alike by the producers and the MMA warp; a slot is released by a tcgen05.commit
@@ -141,33 +142,7 @@ __device__ __forceinline__ void umma_ts_lohi(uint32_t d_tmem, uint32_t a_tmem, u
         : "memory");
 }
 
-constexpr float kSumLimit = 8192.f;                       // a 32-column chunk's row sum above 2^13 triggers a rescale
-
-// Rare path of the single-pass softmax (kept out of line so the hot loop stays small): multiply this row's O
-// accumulator (o_chunks x 32 columns) and the first p_chunks 16-column packed-bf16 P chunks of the current tile by f,
-// an exact power of two.
-__device__ __noinline__ void rescale_tile(uint32_t tS, uint32_t tO, int p_chunks, int o_chunks, float f) {
-    for (int ch = 0; ch < o_chunks; ++ch) {
-        uint32_t o[32];
-        tmem_ld32(tO + 32u * ch, o);
-        tmem_wait_ld();
-#pragma unroll
-        for (int e = 0; e < 32; ++e) o[e] = __float_as_uint(__uint_as_float(o[e]) * f);
-        tmem_st32(tO + 32u * ch, o);
-    }
-    for (int c0 = 0; c0 < p_chunks; ++c0) {
-        uint32_t pw16[16];
-        tmem_ld16(tS + 16u * c0, pw16);
-        tmem_wait_ld();
-#pragma unroll
-        for (int e = 0; e < 16; ++e) {
-            const float lo = __uint_as_float(pw16[e] << 16) * f, hi = __uint_as_float(pw16[e] & 0xffff0000u) * f;
-            pw16[e] = pack_bf16x2(lo, hi);
-        }
-        tmem_st16(tS + 16u * c0, pw16);
-    }
-    tmem_wait_st();
-}
+constexpr float kSumLimit = 8192.f;                       // a 64-column half row summing above 2 * 2^13 sends the tile through the careful pass
 
 template <int D>
 __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams p) {
