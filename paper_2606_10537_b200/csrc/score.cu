@@ -244,6 +244,22 @@ score_kernel(const ScoreParams p, const __grid_constant__ CUtensorMap tmap128, c
                     tc_fence_before();
                     mbar_arrive(s_free(buf));
                     l += tsum;
+                } else if (valid == 1) {
+                    // the one-row tail of a C = 2^k chunk (Cp = C + 1 with the BOS row): a single column, taken by the
+                    // threads of column half 0 alone
+                    if (half == 0) {
+                        const uint32_t xv = tmem_ld1(tS);
+                        tmem_wait_ld();
+                        const float x2 = __uint_as_float(xv) * p.c2;
+                        tc_fence_before();
+                        mbar_arrive(s_free(buf));
+                        const float m_new = fmaxf(m_ref, x2);
+                        l = l * ex2_approx(m_ref - m_new) + ex2_approx(x2 - m_new);
+                        m_ref = m_new;
+                    } else {
+                        tc_fence_before();
+                        mbar_arrive(s_free(buf));
+                    }
                 } else {
                     // ragged tail tile of the chunk: online update per 32-column block with column masks
                     const int mine = max(0, min(64, valid - 64 * half));       // valid columns of this thread's half
