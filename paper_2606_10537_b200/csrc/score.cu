@@ -182,24 +182,24 @@ score_kernel(const ScoreParams p, const __grid_constant__ CUtensorMap tmap128, c
             // sum over 32 columns of 2^(c2*x - m_ref): packed f32x2 arithmetic, exponentials on the MUFU pipe
             auto block_sum = [&](const uint32_t(&v)[32]) {
                 const uint64_t c2v = pack_f32x2(p.c2, p.c2), mv = pack_f32x2(-m_ref, -m_ref);
-                float s0 = 0.f, s1 = 0.f, s2 = 0.f, s3 = 0.f;
+                uint64_t acc0 = 0ull, acc1 = 0ull;
 #pragma unroll
                 for (int e = 0; e < 32; e += 4) {
-                    float x0, x1, x2, x3;
+                    float x0, x1, x2, x3, p0, p1;
                     unpack_f32x2(fma_f32x2(pack_u32x2(v[e], v[e + 1]), c2v, mv), x0, x1);
                     unpack_f32x2(fma_f32x2(pack_u32x2(v[e + 2], v[e + 3]), c2v, mv), x2, x3);
-                    if ((e & 4) == 0 && kPolyShare) {     // a quarter of the exponentials run on the FMA pipe
-                        float r0, r1;
-                        ex2_poly_x2(x0, x1, r0, r1);
-                        s0 += r0;
-                        s1 += r1;
+                    if ((e & 4) == 0 && kPolyShare) {     // a share of the exponentials runs on the FMA pipe
+                        ex2_poly_x2(x0, x1, p0, p1);
                     } else {
-                        s0 += ex2_approx(x0);
-                        s1 += ex2_approx(x1);
+                        p0 = ex2_approx(x0);
+                        p1 = ex2_approx(x1);
                     }
-                    s2 += ex2_approx(x2);
-                    s3 += ex2_approx(x3);
+                    acc0 = add_f32x2(acc0, pack_f32x2(p0, p1));
+                    acc1 = add_f32x2(acc1, pack_f32x2(ex2_approx(x2), ex2_approx(x3)));
                 }
+                float s0, s1, s2, s3;
+                unpack_f32x2(acc0, s0, s1);
+                unpack_f32x2(acc1, s2, s3);
                 return (s0 + s1) + (s2 + s3);
             };
             for (int tt = 0; tt < tiles_per_chunk; ++tt, ++q) {
