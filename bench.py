@@ -42,8 +42,8 @@ FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustain
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture
 # (profiles/), keyed by (workload, kernel); None until a capture exists for that pair.
 NCU_TRAFFIC_BYTES = {
-    # profiles/r1_ncu_full_v5.md (final kernels of round 1)
-    ("sparse32k", "score_kernel"): 1081.384e6 + 3.404032e6,
+    # profiles/r1_ncu_full_v6.md (final kernels of round 1)
+    ("sparse32k", "score_kernel"): 1081.260e6 + 3.529472e6,
     ("sparse32k", "attn_kernel"): 149.460e6 + 5.651712e6,
 }
 
