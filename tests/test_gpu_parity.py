@@ -2,6 +2,8 @@
 inputs.  Bars (SURVEY 8(c) R12 / BASELINE.json north_star): chunk ids and gather indices bit-exact;
 O within 2e-2 + 1e-2|ref| per element and max|d|/max|ref| <= 1e-2; LSE and scores within 1e-3.
 """
+import dataclasses
+
 import numpy as np
 import pytest
 import torch
@@ -109,11 +111,14 @@ def test_scores(B, name, kw):
 
 
 # --------------------------------------------------------------------------- a3+a4+a5 attention
-def _attn_case(B, w, inp, splits, ids=None):
+def _attn_case(B, w, inp, splits, ids=None, scale=None):
     dev = to_device(inp)
     ids = inp["planted"] if ids is None else ids
-    shape = shape_of(inp, ids.shape[-1], w.L_q)
-    O_ref, LSE_ref = oracle.attn(inp["Q_dec"], inp["Kcache"], inp["Vcache"], ids, inp["keep"], inp["K_dec"], inp["V_dec"])
+    shape = shape_of(inp, ids.shape[-1], min(w.L_q, inp["Q_dec"].shape[2]))
+    if scale is not None:
+        shape = dataclasses.replace(shape, scale=scale)
+    O_ref, LSE_ref = oracle.attn(inp["Q_dec"], inp["Kcache"], inp["Vcache"], ids, inp["keep"], inp["K_dec"], inp["V_dec"],
+                                 scale=scale)
     gi_ref = oracle.gather_idx(ids, inp["keep"], w.N, w.C)
     for S in splits:
         gi = torch.empty(gi_ref.shape, dtype=torch.int32, device="cuda")
@@ -183,9 +188,10 @@ def test_step_tiny(B):
         check_close(out["LSE"], ref["LSE"], LSE_ABS)
 
 
-def test_step_sparse32k_full_size_sampled(B):
-    """BASELINE configs[3] at full size in bench.py's launch configuration (n_splits = 0); the oracle
-    checks sampled (b, head) slices one by one."""
+def test_step_sparse32k_full_size_all_heads(B):
+    """BASELINE configs[3] at full size in bench.py's launch configuration (n_splits = 0): scores, chunk ids,
+    gather indices, O and LSE of ALL 128 (b, head) groups against the oracle's own step (ids from
+    oracle.topk(oracle.scores), not from the generator's planted list)."""
     w, inp = _inputs("sparse32k")
     dev = to_device(inp)
     shape = B.Shape.of(w)
@@ -193,20 +199,13 @@ def test_step_sparse32k_full_size_sampled(B):
     out = B.step(shape, dev["Q_dec"], dev["Kcache"], dev["Vcache"], dev["keep"], dev["K_dec"], dev["V_dec"],
                  n_splits=0, gather_idx_out=gi)
     torch.cuda.synchronize()
-    check_exact(out["chunk_ids"], inp["planted"], "planted chunks (all heads)")
-    r = np.random.default_rng(7)
-    sample = [(0, 0), (w.B - 1, w.H - 1)] + [(int(r.integers(w.B)), int(r.integers(w.H))) for _ in range(6)]
-    for b, h in sample:
-        sl = lambda a: a[b:b + 1, h:h + 1]
-        sc = oracle.scores(sl(inp["Q_dec"]), sl(inp["Kcache"]), w.L_q)
-        ids = oracle.topk(sc, w.K)
-        check_close(out["scores"][b:b + 1, h:h + 1], sc, SCORE_ABS, what=f"scores[{b},{h}]")
-        check_exact(out["chunk_ids"][b:b + 1, h:h + 1], ids, f"ids[{b},{h}]")
-        check_exact(gi[b:b + 1, h:h + 1], oracle.gather_idx(ids, sl(inp["keep"]), w.N, w.C), f"gather_idx[{b},{h}]")
-        O_ref, LSE_ref = oracle.attn(sl(inp["Q_dec"]), sl(inp["Kcache"]), sl(inp["Vcache"]), ids, sl(inp["keep"]),
-                                     sl(inp["K_dec"]), sl(inp["V_dec"]))
-        check_O(out["O"][b:b + 1, h:h + 1], O_ref, what=f"O[{b},{h}]")
-        check_close(out["LSE"][b:b + 1, h:h + 1], LSE_ref, LSE_ABS, what=f"LSE[{b},{h}]")
+    ref = oracle.step(inp["Q_dec"], inp["Kcache"], inp["Vcache"], inp["keep"], inp["K_dec"], inp["V_dec"], w.K, w.L_q)
+    check_close(out["scores"], ref["scores"], SCORE_ABS, what="scores")
+    check_exact(out["chunk_ids"], ref["ids"], "chunk ids vs oracle top-K")
+    check_exact(gi, ref["gather_idx"], "gather_idx")
+    check_O(out["O"], ref["O"], what="O (all heads)")
+    check_close(out["LSE"], ref["LSE"], LSE_ABS, what="LSE (all heads)")
+    check_exact(out["chunk_ids"], inp["planted"], "planted chunks (generator sanity)")
 
 
 def test_step_host_matches_step(B):
@@ -354,3 +353,62 @@ def test_attn_ragged_tail_widths(B, tail):
     w, inp = _inputs("tiny", C=100, K=2, keep=1.0, L_q=40, L_d=L_s - 40, H=2, H_kv=2, d=128)
     assert (w.K * (w.C + 1) + w.L) % 128 == tail
     _attn_case(B, w, inp, [1, 2])
+
+
+# --------------------------------------------------------------------------- paths the ABI accepts that round 1 never ran
+@pytest.mark.parametrize("kw", [
+    dict(N=80, C=20, K=40, keep=0.5, d=64, L_q=16, L_d=48),                     # K in 33..64: chunk ids in the second id register
+    dict(N=70, C=12, K=64, keep=1.0, d=128, H=4, H_kv=2, L_q=16, L_d=40),       # K = 64 (the bound), GQA, no keep list
+    dict(N=64, C=30, K=33, keep=0.3, d=128, H=2, H_kv=2, L_q=100, L_d=200),     # K = 33, pair + single items
+])
+def test_attn_many_chunks(B, kw):
+    w, inp = _inputs("tiny", **kw)
+    _attn_case(B, w, inp, [1, 3, 0])
+
+
+@pytest.mark.parametrize("L,L_s", [(32, 96), (96, 32), (1, 200), (130, 7)])
+def test_attn_rows_differ_from_decode_kv_rows(B, L, L_s):
+    """R8's strict shape: only the L = L_d response rows attend while K_dec / V_dec hold the L_s = L_q + L_d
+    query + response rows; and the converse (L_s < L)."""
+    big = max(L, L_s)
+    w, inp = _inputs("tiny", C=150, K=3, keep=0.6, d=128, H=4, H_kv=2, L_q=16, L_d=big - 16)
+    inp["Q_dec"] = np.ascontiguousarray(inp["Q_dec"][:, :, :L])
+    inp["K_dec"] = np.ascontiguousarray(inp["K_dec"][:, :, :L_s])
+    inp["V_dec"] = np.ascontiguousarray(inp["V_dec"][:, :, :L_s])
+    _attn_case(B, w, inp, [1, 2, 0])
+
+
+@pytest.mark.parametrize("scale", [0.05, 0.3])
+def test_attn_explicit_scale(B, scale):
+    w, inp = _inputs("tiny", C=200, K=3, keep=1.0, d=128, L_q=40, L_d=120)
+    _attn_case(B, w, inp, [1, 2], scale=scale)
+
+
+def test_step_explicit_scale_and_strict_rows(B):
+    """pdllm_step with scale = 0.05 (scores, ids and attention all take it)."""
+    w, inp = _inputs("tiny", C=200, H=8, H_kv=4, d=128, L_q=24, L_d=40)
+    dev = to_device(inp)
+    shape = dataclasses.replace(B.Shape.of(w), scale=0.05)
+    ref = oracle.step(inp["Q_dec"], inp["Kcache"], inp["Vcache"], inp["keep"], inp["K_dec"], inp["V_dec"], w.K, w.L_q,
+                      scale=0.05)
+    out = B.step(shape, dev["Q_dec"], dev["Kcache"], dev["Vcache"], dev["keep"], dev["K_dec"], dev["V_dec"], n_splits=2)
+    torch.cuda.synchronize()
+    check_close(out["scores"], ref["scores"], SCORE_ABS, what="scores")
+    check_exact(out["chunk_ids"], ref["ids"])
+    check_O(out["O"], ref["O"])
+    check_close(out["LSE"], ref["LSE"], LSE_ABS)
+
+
+@pytest.mark.parametrize("kw", [
+    dict(B=5, H=8, H_kv=8, d=64, N=512, C=31, K=4, L_q=16, L_d=8),     # 40 groups x 512 chunks: 69 units per CTA, runs cross
+                                                                       # 64-chunk segments and (b, g) boundaries (P:231: N = 512)
+    dict(B=2, H=64, H_kv=64, d=128, N=256, C=15, K=4, L_q=8, L_d=8),   # 128 groups x 256 chunks, one 16-row tile per chunk
+    dict(B=1, H=12, H_kv=4, d=64, N=2000, C=12, K=5, L_q=100, L_d=4),  # GQA G = 3: 300 scoring rows = 3 M tiles, 81 units per CTA
+])
+def test_scores_long_cta_runs(B, kw):
+    w, inp = _inputs("tiny", **kw)
+    shape = B.Shape.of(w)
+    got = B.score_chunks(shape, dev_bf16(inp["Q_dec"]), dev_bf16(inp["Kcache"]))
+    ref = oracle.scores(inp["Q_dec"], inp["Kcache"], w.L_q)
+    check_close(got, ref, SCORE_ABS, what="scores (long CTA runs)")
+    check_exact(B.select_topk(shape, got), oracle.topk(ref, w.K))
