@@ -19,7 +19,9 @@
  *   - extern "C"; returns int: 0 = PDLLM_OK, < 0 = error (see pdllm_status).
  *   - ENQUEUE-ONLY on the given stream: never synchronises, never allocates or
  *     frees device memory, keeps no state between calls (TMA descriptors are
- *     passed to kernels by value).
+ *     passed to kernels by value; the only thing the library remembers is the
+ *     SM count of each device, an immutable hardware fact read on first use;
+ *     launches set the kernels' dynamic shared-memory attribute each call).
  *   - "device" pointers are caller-owned device memory (e.g. a torch allocation),
  *     16-byte aligned, dense row-major in the stated shape; inputs are read-only;
  *     outputs are fully overwritten; buffers must stay alive until the stream has
@@ -27,7 +29,16 @@
  *   - Validation is host-side only (null pointer, misalignment, unsupported shape,
  *     workspace too small): the call returns an error and enqueues nothing.
  *     Device-side data errors (chunk id outside [0,N), keep slot outside [0,C],
- *     unsorted keep list) are undefined behaviour.
+ *     unsorted keep list, keep[..,0] != 0) are undefined behaviour in normal
+ *     operation: the kernels address the cache with 32-bit offsets formed from them.
+ *   - DEBUG SWITCH: with the environment variable PDLLM_DEBUG_VALIDATE=1 the calls
+ *     that take chunk_ids / token_keep_idx (pdllm_gather_idx, pdllm_sparse_attn,
+ *     pdllm_step*, pdllm_compact_kv, pdllm_score_tokens consumers) first run a
+ *     checking kernel over those lists on `stream`, SYNCHRONISE the stream, and
+ *     return PDLLM_ERR_DATA with nothing else enqueued on the first violation
+ *     (this mode allocates and frees a 4-byte device flag per call: the one
+ *     exception to the rules above; for pdllm_step* the ids are produced
+ *     internally, so only the keep list is checked).
  *   - bf16 = IEEE bfloat16 bit patterns; O is rounded to bf16 round-to-nearest-even
  *     from the fp32 accumulator (R11).
  *   - GQA: query head h reads KV head h / (H / H_kv) (R4).
@@ -54,7 +65,8 @@ typedef enum {
     PDLLM_ERR_SHAPE = -3,       /* a shape field is out of range (see pdllm_shape) */
     PDLLM_ERR_WORKSPACE = -4,   /* workspace_bytes smaller than pdllm_workspace_bytes() */
     PDLLM_ERR_UNSUPPORTED = -5, /* valid request that this build does not implement */
-    PDLLM_ERR_CUDA = -6         /* a CUDA runtime / driver call or a launch failed */
+    PDLLM_ERR_CUDA = -6,        /* a CUDA runtime / driver call or a launch failed */
+    PDLLM_ERR_DATA = -7         /* PDLLM_DEBUG_VALIDATE=1 only: a device-side index list is malformed */
 } pdllm_status;
 
 /* Shapes shared by all calls (S8 symbols).
@@ -81,8 +93,13 @@ int pdllm_version(void);                       /* e.g. 100 = 0.1.0 */
 const char *pdllm_strerror(int status);        /* static string, never NULL */
 
 /* a6 (S8(a); P:189-191 fixes S = 4, NS: "chosen from N*K*C and the number of
- * SMs"): smallest split count that gives about one wave of CTAs on num_sms SMs
- * while leaving every split at least two 128-row KV tiles.  >= 1. */
+ * SMs"): the split count a cost model of the persistent attention kernel picks
+ * for num_sms SMs (<= 0: the current device's count).  Per candidate S in
+ * 1..min(KV tiles, 64) the model takes the busiest CTA's KV-tile steps under the
+ * kernel's item order (plus a fixed cost per work item) and, for S > 1, the
+ * combine step's launch and its 2*S*rows*d*4 bytes of partial traffic; the
+ * cheapest S wins, a larger S only by a 3 % margin.  A split may be a single
+ * 128-row KV tile; never more splits than KV tiles.  >= 1. */
 int32_t pdllm_auto_splits(const pdllm_shape *shape, int32_t num_sms);
 
 /* Bytes of scratch pdllm_sparse_attn / pdllm_step need for n_splits splits
@@ -187,19 +204,28 @@ int pdllm_step_profiled(const pdllm_shape *shape, const void *Q_dec, const void 
  * changes every step is the decode block.  This call enqueues, on `stream`:
  * the H2D copy of h_Q_dec (host, pinned for true async) into d_scratch, the
  * steps of pdllm_step, and D2H copies of O, LSE and chunk ids into the host
- * outputs.  h_K_dec / h_V_dec, which only the attention reads, are copied on a
- * side stream the library owns (one per host thread and device, created on
- * first use): it forks from `stream` at the start of the call and joins it
- * ahead of the attention kernel, so those copies run under the scoring kernel;
- * to the caller all work is ordered on `stream`, which it synchronises before
- * reading the outputs.
+ * outputs.  h_K_dec / h_V_dec are read by the attention only: when the caller
+ * passes a side stream (`side` != NULL: a second stream of the same device and
+ * two events created with cudaEventDisableTiming, all caller-owned; the library
+ * creates and keeps nothing) they are copied on it -- the side stream forks from
+ * `stream` at the start of the call and joins it ahead of the attention kernel,
+ * so those copies run under the scoring kernel.  side == NULL: every copy goes
+ * on `stream` in order.  To the caller all work is ordered on `stream`, which it
+ * synchronises before reading the outputs.
  *   d_scratch  device scratch of >= pdllm_step_host_scratch_bytes() bytes; one
  *              call at a time may use it                                          */
+typedef struct {
+    pdllm_stream_t stream;   /* the side stream */
+    void *ev_fork;           /* cudaEvent_t, recorded on `stream`, waited on by the side stream */
+    void *ev_join;           /* cudaEvent_t, recorded on the side stream, waited on by `stream` */
+} pdllm_side_stream;
+
 int pdllm_step_host(const pdllm_shape *shape, const void *h_Q_dec, const void *h_K_dec,
                     const void *h_V_dec, const void *d_Kcache, const void *d_Vcache,
                     const int32_t *d_token_keep_idx, int32_t n_splits,
                     void *h_O, float *h_LSE, int32_t *h_chunk_ids,
-                    void *d_scratch, size_t scratch_bytes, pdllm_stream_t stream);
+                    void *d_scratch, size_t scratch_bytes,
+                    const pdllm_side_stream *side, pdllm_stream_t stream);
 
 #ifdef __cplusplus
 }

@@ -29,6 +29,10 @@ class PdllmShape(ctypes.Structure):
         ("scale", ctypes.c_float)]
 
 
+class PdllmSideStream(ctypes.Structure):
+    _fields_ = [(n, ctypes.c_void_p) for n in ("stream", "ev_fork", "ev_join")]
+
+
 class PdllmStageEvents(ctypes.Structure):
     _fields_ = [(n, ctypes.c_void_p) for n in ("begin", "after_score", "after_topk", "after_attn", "end")]
 
@@ -93,7 +97,7 @@ def lib() -> ctypes.CDLL:
     L.pdllm_step.argtypes = [shp, vp, vp, vp, vp, vp, vp, i32, vp, vp, vp, vp, vp, vp, sz, vp]
     L.pdllm_step_profiled.argtypes = [shp, vp, vp, vp, vp, vp, vp, i32, vp, vp, vp, vp, vp, vp, sz,
                                       ctypes.POINTER(PdllmStageEvents), vp]
-    L.pdllm_step_host.argtypes = [shp, vp, vp, vp, vp, vp, vp, i32, vp, vp, vp, vp, sz, vp]
+    L.pdllm_step_host.argtypes = [shp, vp, vp, vp, vp, vp, vp, i32, vp, vp, vp, vp, sz, ctypes.POINTER(PdllmSideStream), vp]
     for n in ("pdllm_score_chunks", "pdllm_select_topk", "pdllm_gather_idx", "pdllm_sparse_attn", "pdllm_lse_combine",
               "pdllm_step", "pdllm_step_profiled", "pdllm_step_host"):
         getattr(L, n).restype = ctypes.c_int
@@ -235,9 +239,25 @@ def step(shape: Shape, Q_dec, Kcache, Vcache, token_keep_idx, K_dec, V_dec, n_sp
     return dict(scores=scores, chunk_ids=chunk_ids, O=O, LSE=LSE)
 
 
+class SideStream:
+    """A caller-owned side stream + fork / join events for step_host (the library keeps none of its own)."""
+
+    def __init__(self, device=None):
+        torch = _torch()
+        self.stream = torch.cuda.Stream(device=device)
+        self.ev_fork, self.ev_join = torch.cuda.Event(), torch.cuda.Event()
+        for e in (self.ev_fork, self.ev_join):      # torch creates the cudaEvent_t on first record
+            e.record(self.stream)
+
+    def c(self) -> PdllmSideStream:
+        return PdllmSideStream(self.stream.cuda_stream, self.ev_fork.cuda_event, self.ev_join.cuda_event)
+
+
 def step_host(shape: Shape, h_Q_dec, h_K_dec, h_V_dec, d_Kcache, d_Vcache, d_token_keep_idx, n_splits, h_O, h_LSE,
-              h_chunk_ids, d_scratch, stream=None):
-    """pdllm_step with HOST (pinned) per-step tensors: H2D copies, the step, D2H copies, all enqueued on `stream`."""
+              h_chunk_ids, d_scratch, side: "SideStream | None" = None, stream=None):
+    """pdllm_step with HOST (pinned) per-step tensors: H2D copies, the step, D2H copies, all ordered on `stream`;
+    with `side` the K_dec / V_dec copies run on that stream underneath the scoring kernel."""
+    sd = ctypes.byref(side.c()) if side is not None else None
     _check(lib().pdllm_step_host(ctypes.byref(shape.c()), _ptr(h_Q_dec), _ptr(h_K_dec), _ptr(h_V_dec), _ptr(d_Kcache),
                                  _ptr(d_Vcache), _ptr(d_token_keep_idx), n_splits, _ptr(h_O), _ptr(h_LSE),
-                                 _ptr(h_chunk_ids), _ptr(d_scratch), d_scratch.numel(), _stream(stream)))
+                                 _ptr(h_chunk_ids), _ptr(d_scratch), d_scratch.numel(), sd, _stream(stream)))

@@ -25,30 +25,6 @@
 #include "pdllm_internal.h"
 #include "ptx.cuh"
 
-#ifdef PDLLM_TRACE
-// Perf-debug build only (-DPDLLM_TRACE, never the shipped library): one CTA logs (clock64, code, arg) per role.
-__device__ long long *g_pdllm_trace = nullptr;
-__device__ int g_pdllm_trace_cta = 0;
-extern "C" int pdllm_debug_set_trace(void *dev_buf) {
-    return (int)cudaMemcpyToSymbol(g_pdllm_trace, &dev_buf, sizeof(void *));
-}
-extern "C" int pdllm_debug_set_trace_cta(int cta) {
-    return (int)cudaMemcpyToSymbol(g_pdllm_trace_cta, &cta, sizeof(int));
-}
-#define PDLLM_TRACE_DECL(role) \
-    longlong2 *tr_p = ((int)blockIdx.x == g_pdllm_trace_cta && g_pdllm_trace) ? reinterpret_cast<longlong2 *>(g_pdllm_trace) + (role) * 4096 : nullptr; \
-    longlong2 *const tr_end = tr_p + 4096;
-#define PDLLM_TR(code, arg)                                                                       \
-    do {                                                                                          \
-        if (tr_p && tr_p < tr_end) {                                                              \
-            *tr_p++ = make_longlong2(clock64(), ((long long)(code) << 32) | (unsigned)(arg));     \
-        }                                                                                         \
-    } while (0)
-#else
-#define PDLLM_TRACE_DECL(role)
-#define PDLLM_TR(code, arg)
-#endif
-
 namespace pdllm {
 
 namespace {
@@ -57,7 +33,9 @@ constexpr int kSoftmaxThreads = 128;                      // per stream
 constexpr int kProducerThreads = 128;
 constexpr int kProducerWarp0 = 8;
 constexpr int kMmaWarp0 = 12;
-constexpr int kAttnThreads = 2 * kSoftmaxThreads + kProducerThreads + 32;
+constexpr int kAttnThreads = 2 * kSoftmaxThreads + kProducerThreads + 128;     // 16 warps: whole warpgroups for setmaxnreg
+// register budgets after the roles part ways (setmaxnreg; 256 * 176 + 128 * 104 + 128 * 56 = 65536)
+constexpr int kSoftmaxRegs = 176, kProducerRegs = 104, kOtherRegs = 56;
 constexpr int kInvalidRow = INT32_MIN;
 constexpr float kRescaleThreshold = 8.0f;                 // log2 units: P stays <= 2^8 between reference-max updates
 
@@ -142,7 +120,13 @@ __device__ __forceinline__ void umma_ts_lohi(uint32_t d_tmem, uint32_t a_tmem, u
         : "memory");
 }
 
-constexpr float kSumLimit = 8192.f;                       // a 64-column half row summing above 2 * 2^13 sends the tile through the careful pass
+constexpr float kSoftLimit = 16384.f;                     // 2^14: a row sum beyond it raises the reference ahead of the next tile
+constexpr float kHardLimit = 1.2676506e30f;               // 2^100: beyond it (or inf / NaN) the tile is redone carefully
+
+template <int N>
+__device__ __forceinline__ void setmaxnreg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
+template <int N>
+__device__ __forceinline__ void setmaxnreg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
 
 template <int D>
 __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams p) {
@@ -162,7 +146,7 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
     __shared__ uint64_t bars[BAR_KV + 2 * (ST + 1)];
     __shared__ uint32_t tmem_slot;
     __shared__ int32_t s_items[4];                        // the CTA's next work items (ring, published by the producers)
-    __shared__ float s_x[kTileM][2];                      // per-row exchange slots of the two column halves
+    __shared__ float s_ml[kSoftmaxThreads][3];            // single items: stream 1's (m_ref, l, O scale) for the in-CTA merge
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const uint32_t bar0 = smem_u32(&bars[0]);
@@ -176,9 +160,9 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
         mbar_init(bar(BAR_QFREE), 1);
         for (int s = 0; s < 2; ++s) {
             mbar_init(bar(BAR_SREADY0 + s), 1);
-            mbar_init(bar(BAR_PREADY0 + s), 2 * kSoftmaxThreads);
+            mbar_init(bar(BAR_PREADY0 + s), kSoftmaxThreads);
             mbar_init(bar(BAR_OREADY0 + s), 1);
-            mbar_init(bar(BAR_OFREE0 + s), 2 * kSoftmaxThreads);
+            mbar_init(bar(BAR_OFREE0 + s), kSoftmaxThreads);
         }
         for (int s = 0; s <= ST; ++s) {
             mbar_init(kv_full(s), kProducerThreads);
@@ -197,6 +181,7 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
 
     if (warp >= kProducerWarp0 && warp < kMmaWarp0) {
         // =============================== producers: index-driven gather ===============================
+        setmaxnreg_dec<kProducerRegs>();
         const int pt = tid - kProducerWarp0 * 32, pw = pt >> 5;
         const int rsub = lane / kChunksPerRow, c = lane % kChunksPerRow;
         const uint32_t dst_pc = (uint32_t)(c >> 3) * Cfg::kPanelBytes;
@@ -254,7 +239,6 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
         int cur = 0;
         uint32_t free_bits = (1u << (ST + 1)) - 1u;
         int n_done = 0;                                   // items finished by this CTA
-        PDLLM_TRACE_DECL(0)
         // Work items are handed out dynamically (costliest first: pair items, then single items), so CTAs that
         // finish early take more; thread 0 of the producers fetches, the other roles follow through s_items.
         for (;; ++n_done) {
@@ -348,12 +332,9 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
                 load_q();                                 // Q first: its rows need no indices, the first tile's are in flight
                 for (int jt = 0; jt < it.nt; ++jt) {
                     const int my_idx = nx_base + nx_raw;
-                    if (pt == 0) PDLLM_TR(10, jt);
                     if (jt + 1 < it.nt) prefetch_index(it.t0 + jt + 1);         // in flight while this tile is issued
                     const int slot_k = take_slot(), slot_v = take_slot();
-                    if (pt == 0) PDLLM_TR(11, jt);
                     load_tile(it.t0 + jt, my_idx, sKV(slot_k), sKV(slot_v), true, true);
-                    if (pt == 0) PDLLM_TR(12, jt);
                     publish(kv_full(slot_k));
                     publish(kv_full(slot_v));
                 }
@@ -361,12 +342,9 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
                 // one tile per load, in the MMA warp's consumption order K(t0); { K(t0+i+1), V(t0+i) }; V(t0+nt-1)
                 // (each tile has a single user); a tile's indices are computed once and serve its K and its V load
                 auto load_one = [&](int tile, int idx, bool is_v) {
-                    if (pt == 0) PDLLM_TR(10, tile);
                     const int slot = take_slot();
-                    if (pt == 0) PDLLM_TR(11, tile);
                     const uint32_t dst = sKV(slot);
                     load_tile(tile, idx, dst, dst, !is_v, is_v);
-                    if (pt == 0) PDLLM_TR(12, tile);
                     publish(kv_full(slot));
                 };
                 prefetch_index(it.t0);
@@ -386,11 +364,11 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
         }
     } else if (warp == kMmaWarp0) {
         // =============================== MMA issuer ===============================
+        setmaxnreg_dec<kOtherRegs>();
         // One warp issues both streams' MMAs in the fixed order QK(0,0) QK(1,0) { PV(0,j) QK(0,j+1) PV(1,j) QK(1,j+1) }:
         // the in-order tensor pipe then keeps the two softmax streams in anti-phase (one stream's exponentials run
         // under the other stream's MMAs).  The warp stays converged (all lanes wait on the barriers); one elected
         // lane issues the tcgen05 instructions, so the descriptors stay in uniform registers.
-        PDLLM_TRACE_DECL(1)
         int cur = 0;                                      // ring cursor / phase bits, mirrored from the producers
         uint32_t full_bits = 0u;
         uint32_t n_pready[2] = {0, 0}, n_oready[2] = {0, 0};
@@ -457,34 +435,26 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
                     // the loads this stream step needs have normally landed long ago: cross them into the async proxy
                     // BEFORE waiting for P, so that P*V and the next Q*K^T issue back to back once P is there
                     if (fresh) {
-                        if (lane == 0) PDLLM_TR(27, j);
                         v_slot = next_load();
                         if (has_next) k_slot = next_load();
-                        if (lane == 0) PDLLM_TR(28, j);
                         fence_proxy_async_smem();
-                        if (lane == 0) PDLLM_TR(29, j);
                     }
-                    if (lane == 0) PDLLM_TR(23, s);
                     mbar_wait(bar(BAR_PREADY0 + s), n_pready[s]++ & 1u);
                     if (j == 0 && n_oready[s] > 0) mbar_wait(bar(BAR_OFREE0 + s), (n_oready[s] - 1) & 1u);
                     tc_fence_after();
-                    if (lane == 0) PDLLM_TR(25, s);
                     const int ksteps = (int)(n_mma_of(tile) >> 4);
                     if (elect_one()) {
-                        // 16 kv rows per step: A = 8 TMEM columns of packed bf16 P (column half h of the tile keeps its P at
-                        // S columns 64h..64h+31), B = 16 V rows (MN-major, 2048 B)
+                        // 16 kv rows per step: A = 8 TMEM columns of packed bf16 P, B = 16 V rows (MN-major, 2048 B)
                         const int slot = v_slot;
                         const uint32_t v_lo = lo_v | ((sKV(slot) & 0x3FFFFu) >> 4);
                         const uint32_t tS = tmem + 128u * s, tO = tmem + kOCol + 128u * s;
                         if (ksteps == kTileN / 16) {
 #pragma unroll
                             for (int ks = 0; ks < kTileN / 16; ++ks)
-                                umma_ts_lohi(tO, tS + 64u * (ks >> 2) + 8u * (ks & 3), v_lo + 128u * ks, hi_v, idesc_pv,
-                                             (j > 0 || ks > 0) ? 1u : 0u);
+                                umma_ts_lohi(tO, tS + 8u * ks, v_lo + 128u * ks, hi_v, idesc_pv, (j > 0 || ks > 0) ? 1u : 0u);
                         } else {
                             for (int ks = 0; ks < ksteps; ++ks)
-                                umma_ts_lohi(tO, tS + 64u * (ks >> 2) + 8u * (ks & 3), v_lo + 128u * ks, hi_v, idesc_pv,
-                                             (j > 0 || ks > 0) ? 1u : 0u);
+                                umma_ts_lohi(tO, tS + 8u * ks, v_lo + 128u * ks, hi_v, idesc_pv, (j > 0 || ks > 0) ? 1u : 0u);
                         }
                         if (release) umma_commit(kv_free(slot));
                         if (last_pv) umma_commit(bar(BAR_OREADY0 + s));
@@ -492,262 +462,237 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
                     }
                     __syncwarp();
                     if (last_pv) ++n_oready[s];
-                    if (lane == 0) PDLLM_TR(26, s);
                 }
             }
         }
-    } else {
-        // =============================== softmax (two threads per query row, both streams) ===============================
-        // A warp may only touch TMEM lanes 32*(warp%4)..+31 and warps w, w+4 sit on the same SM sub-partition, where a
-        // lone warp reaches only half the MUFU rate (measured: 590 clk per 32-column block alone, 352 clk each for two
-        // warps side by side).  So a query row is shared by two threads: half h = warp/4 owns columns 64h..64h+63 of
-        // every S tile (and columns D/2*h.. of the row's O accumulators), and the eight warps work through the tiles of
-        // BOTH streams in the order the MMA warp produces them: S(0,j), S(1,j), S(0,j+1), ...  Both halves use one
-        // reference max per row (P*V accumulates the whole row); their row sums are kept apart and added in the epilogue.
-        // P (packed bf16) goes over the first 32 of the thread's own 64 S columns, so the halves never touch each
-        // other's columns; they meet once per tile on a 64-thread named barrier that carries the overflow vote.
-        const int half = warp >> 2;
-        const int row = (warp & 3) * 32 + lane;
+    } else if (warp < 2 * (kSoftmaxThreads / 32)) {
+        // =============================== softmax (thread = query row, one 4-warp group per stream) ===============================
+        // Warps 0-3 own stream 0, warps 4-7 stream 1 (a warp may only touch TMEM lanes 32*(warp%4)..+31, its 32 rows).
+        // The in-order tensor pipe keeps the two groups in anti-phase: while one group works on its S tile the pipe runs
+        // the other stream's P*V and next Q*K^T.  A thread holds its row's whole 128-column S tile in registers (the
+        // group raises its register budget to kSoftmaxRegs) and keeps a REFERENCE max per row in log2 units: the
+        // stream's first tile fixes it with a max pass, later tiles take ONE pass P = 2^(c2*S - m_ref).  P may outgrow 1:
+        // a tile whose row sum exceeds 2^kSoftOctaves is still exact (bf16 and fp32 carry the exponent) and only raises
+        // the reference, by whole octaves, ahead of the row's NEXT tile, when the O accumulator is at rest -- l and O are
+        // multiplied by an exact power of two.  Only a sum beyond 2^kHardOctaves (a logit more than ~100 octaves above
+        // the reference inside one tile) or a ragged tail tile goes through the careful pass: exact row max first.
+        setmaxnreg_inc<kSoftmaxRegs>();
+        const int s = warp >> 2;                          // stream
+        const int row = tid & (kSoftmaxThreads - 1);
         const uint32_t lane_base = (uint32_t)((warp & 3) * 32) << 16;
-        constexpr int kOHalf = D / 2;                     // O columns per thread
-        const uint32_t pair_bar = 4u + (uint32_t)(warp & 3);
-        uint32_t ph_s = 0u, ph_o = 0u;                    // phase bits of S-ready / O-ready, bit s = stream s
-        PDLLM_TRACE_DECL(2 + half)
-        auto pair_sync = [&]() { asm volatile("bar.sync %0, 64;" ::"r"(pair_bar) : "memory"); };
-        auto pair_any = [&](bool pred) {
-            uint32_t r;
-            asm volatile(
-                "{\n\t.reg .pred p, q;\n\tsetp.ne.u32 p, %2, 0;\n\tbarrier.cta.red.or.pred.aligned q, %1, 64, p;\n\t"
-                "selp.u32 %0, 1, 0, q;\n\t}"
-                : "=r"(r)
-                : "r"(pair_bar), "r"((uint32_t)pred)
-                : "memory");
-            return r != 0;
-        };
-        // both halves' values of a per-row quantity (two pair barriers: publish, then release the slots)
-        auto pair_xch = [&](float v, float &v0, float &v1) {
-            s_x[row][half] = v;
-            pair_sync();
-            v0 = s_x[row][0];
-            v1 = s_x[row][1];
-            pair_sync();
-        };
-        if (row == 0) PDLLM_TR(1, 0);
+        const uint32_t tS = tmem + 128u * s + lane_base, tO = tmem + kOCol + 128u * s + lane_base;
+        uint32_t n_sready = 0, n_oready = 0;
+        int n_modeB = 0;
         for (int n_done = 0;; ++n_done) {
             mbar_wait(bar(BAR_ITEM0 + (n_done & 3)), (uint32_t)(n_done >> 2) & 1u);
             const int ii = s_items[n_done & 3];
-            if (row == 0) PDLLM_TR(2, ii);
             if (ii < 0) break;
             const Item it = decode_item(p, ii);
-            const int ns0 = it.modeA ? it.nt : (it.nt + 1) / 2, ns1 = it.modeA ? it.nt : it.nt / 2;    // tiles per stream
-            if (row == 0) PDLLM_TR(40, ii);
-            float m0 = -INFINITY, m1 = -INFINITY, l0 = 0.f, l1 = 0.f;     // per stream: reference max, this half's row sum
-            for (int j = 0; j < ns0; ++j) {
+            const int n_mine = it.modeA ? it.nt : (s == 0 ? (it.nt + 1) / 2 : it.nt / 2);
+            float m_ref = -INFINITY, l = 0.f, pend = 0.f;     // pend: octaves the reference is to be raised by
+            // multiply this row's O accumulator by f (an exact power of two); O is at rest: PV(s, j-1) completed before
+            // S(s, j) was committed
+            auto scale_O = [&](float f) {
 #pragma unroll 1
-                for (int s = 0; s < 2; ++s) {
-                    if (j >= (s ? ns1 : ns0)) continue;
-                    float m_ref = s ? m1 : m0, l = s ? l1 : l0;
-                    const uint32_t tSh = tmem + 128u * s + lane_base + 64u * half;      // this thread's 64 S columns
-                    const uint32_t tOh = tmem + kOCol + 128u * s + lane_base + (uint32_t)(kOHalf * half);
-                    const int tile = it.modeA ? it.t0 + j : it.t0 + 2 * j + s;
-                    const int n_valid = min(kTileN, p.S_kv - tile * kTileN);
-                    if (row == 0) PDLLM_TR(30, 2 * j + s);
-                    mbar_wait(bar(BAR_SREADY0 + s), (ph_s >> s) & 1u);
-                    ph_s ^= 1u << s;
-                    tc_fence_after();
-                    if (row == 0) PDLLM_TR(31, 2 * j + s);
-                    // one 32-column block of a full tile: P = 2^(c2*S - m_ref) as packed bf16 and its row sum; packed
-                    // f32x2 arithmetic (one FFMA2 / FADD2 per two columns), the exponentials on the MUFU pipe
-                    auto chunk_exp = [&](const uint32_t(&v)[32], uint32_t(&w)[16]) {
-                        const uint64_t c2v = pack_f32x2(p.c2, p.c2), mv = pack_f32x2(-m_ref, -m_ref);
-                        uint64_t acc0 = 0ull, acc1 = 0ull;
+                for (int ch = 0; ch < D / 32; ++ch) {
+                    uint32_t o[32];
+                    tmem_ld32(tO + 32u * ch, o);
+                    tmem_wait_ld();
 #pragma unroll
-                        for (int e = 0; e < 32; e += 4) {
-                            float x0, x1, x2, x3;
-                            unpack_f32x2(fma_f32x2(pack_u32x2(v[e], v[e + 1]), c2v, mv), x0, x1);
-                            unpack_f32x2(fma_f32x2(pack_u32x2(v[e + 2], v[e + 3]), c2v, mv), x2, x3);
-                            const float p0 = ex2_approx(x0), p1 = ex2_approx(x1), p2 = ex2_approx(x2), p3 = ex2_approx(x3);
-                            acc0 = add_f32x2(acc0, pack_f32x2(p0, p1));
-                            acc1 = add_f32x2(acc1, pack_f32x2(p2, p3));
-                            w[e >> 1] = pack_bf16x2(p0, p1);
-                            w[(e >> 1) + 1] = pack_bf16x2(p2, p3);
-                        }
-                        float s0, s1, s2, s3;
-                        unpack_f32x2(acc0, s0, s1);
-                        unpack_f32x2(acc1, s2, s3);
-                        return (s0 + s1) + (s2 + s3);
-                    };
-                    bool careful = n_valid != kTileN;
-                    if (!careful && j == 0) {
+                    for (int e = 0; e < 32; ++e) o[e] = __float_as_uint(__uint_as_float(o[e]) * f);
+                    tmem_st32(tO + 32u * ch, o);
+                }
+            };
+            // one 32-column block of a full tile: P = 2^(c2*S - m_ref) as packed bf16 and its row sum; packed f32x2
+            // arithmetic (one FFMA2 / FADD2 per two columns), the exponentials on the MUFU pipe
+            auto chunk_exp = [&](const uint32_t(&v)[32], uint32_t *w) {
+                const uint64_t c2v = pack_f32x2(p.c2, p.c2), mv = pack_f32x2(-m_ref, -m_ref);
+                uint64_t acc0 = 0ull, acc1 = 0ull;
+#pragma unroll
+                for (int e = 0; e < 32; e += 4) {
+                    float x0, x1, x2, x3;
+                    unpack_f32x2(fma_f32x2(pack_u32x2(v[e], v[e + 1]), c2v, mv), x0, x1);
+                    unpack_f32x2(fma_f32x2(pack_u32x2(v[e + 2], v[e + 3]), c2v, mv), x2, x3);
+                    const float p0 = ex2_approx(x0), p1 = ex2_approx(x1), p2 = ex2_approx(x2), p3 = ex2_approx(x3);
+                    acc0 = add_f32x2(acc0, pack_f32x2(p0, p1));
+                    acc1 = add_f32x2(acc1, pack_f32x2(p2, p3));
+                    w[e >> 1] = pack_bf16x2(p0, p1);
+                    w[(e >> 1) + 1] = pack_bf16x2(p2, p3);
+                }
+                float s0, s1, s2, s3;
+                unpack_f32x2(acc0, s0, s1);
+                unpack_f32x2(acc1, s2, s3);
+                return (s0 + s1) + (s2 + s3);
+            };
+            for (int j = 0; j < n_mine; ++j) {
+                const int tile = it.modeA ? it.t0 + j : it.t0 + 2 * j + s;
+                const int n_valid = min(kTileN, p.S_kv - tile * kTileN);
+                mbar_wait(bar(BAR_SREADY0 + s), n_sready++ & 1u);
+                tc_fence_after();
+                if (__any_sync(0xffffffffu, pend > 0.f)) {
+                    // the previous tile's row sum outgrew 2^kSoftOctaves: raise the reference now that O is at rest
+                    const float f = ex2_approx(-pend);                // exact power of two (1 for rows that are fine)
+                    l *= f;
+                    scale_O(f);
+                    tmem_wait_st();
+                    m_ref += pend;
+                    pend = 0.f;
+                }
+                bool careful = n_valid != kTileN;
+                if (!careful) {
+                    uint32_t va[32], vb[32], w[64];
+                    tmem_ld32(tS, va);
+                    tmem_ld32(tS + 32u, vb);
+                    tmem_wait_ld();
+                    if (j == 0) {
                         // first tile of the stream (full): its row max becomes the reference (one extra pass over S)
-                        uint32_t va[32], vb[32];
-                        tmem_ld32(tSh, va);
-                        tmem_ld32(tSh + 32u, vb);
-                        tmem_wait_ld();
+                        uint32_t vc[32], vd[32];
+                        tmem_ld32(tS + 64u, vc);
+                        tmem_ld32(tS + 96u, vd);
                         float mx[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
 #pragma unroll
                         for (int e = 0; e < 32; ++e) mx[e & 3] = fmaxf(mx[e & 3], fmaxf(__uint_as_float(va[e]), __uint_as_float(vb[e])));
-                        float t0, t1;
-                        pair_xch(fmaxf(fmaxf(mx[0], mx[1]), fmaxf(mx[2], mx[3])), t0, t1);
-                        m_ref = fmaxf(t0, t1) * p.c2;
+                        tmem_wait_ld();
+#pragma unroll
+                        for (int e = 0; e < 32; ++e) mx[e & 3] = fmaxf(mx[e & 3], fmaxf(__uint_as_float(vc[e]), __uint_as_float(vd[e])));
+                        m_ref = fmaxf(fmaxf(mx[0], mx[1]), fmaxf(mx[2], mx[3])) * p.c2;
                     }
+                    // single pass against the reference, TMEM loads one block ahead of the arithmetic
+                    uint32_t vc[32];
+                    tmem_ld32(tS + 64u, vc);
+                    float lsum = chunk_exp(va, w);
+                    tmem_wait_ld();
+                    tmem_ld32(tS + 96u, va);
+                    lsum += chunk_exp(vb, w + 16);
+                    tmem_wait_ld();
+                    lsum += chunk_exp(vc, w + 32);
+                    lsum += chunk_exp(va, w + 48);
+                    careful = __any_sync(0xffffffffu, !(lsum <= kHardLimit));       // also catches inf / NaN sums
                     if (!careful) {
-                        // Single pass against the current reference.  The half-row sum doubles as the overflow detector
-                        // (some P > 2^14 implies sum > 2 * kSumLimit); an overflow anywhere in the two warps (rare) sends
-                        // the tile through the careful pass -- nothing has been stored yet, S is intact.
-                        uint32_t va[32], vb[32], w0[16], w1[16];
-                        tmem_ld32(tSh, va);
-                        tmem_wait_ld();
-                        if (row == 0) PDLLM_TR(36, 0);
-                        tmem_ld32(tSh + 32u, vb);
-                        float lsum = chunk_exp(va, w0);
-                        if (row == 0) PDLLM_TR(36, 1);
-                        tmem_wait_ld();
-                        lsum += chunk_exp(vb, w1);
-                        if (row == 0) PDLLM_TR(36, 2);
-                        careful = pair_any(!(lsum <= 2.f * kSumLimit));
-                        if (row == 0) PDLLM_TR(36, 3);
-                        if (!careful) {
-                            l += lsum;
-                            tmem_st16(tSh, w0);
-                            tmem_st16(tSh + 16u, w1);
-                        }
-                        if (row == 0) PDLLM_TR(36, 4);
-                    }
-                    if (careful) {
-                        // Ragged tail tile (possibly the stream's first) or after an overflow vote: row max over the valid
-                        // columns of both halves -> reference (raised by whole octaves once it exists, so that l and O
-                        // rescale exactly) -> masked exponentials -> P.  S is read twice.
-                        const int mine = max(0, min(64, n_valid - 64 * half));          // valid columns of this half
-                        float tmax = -INFINITY;
-#pragma unroll 1
-                        for (int b = 0; b < 2; ++b) {
-                            if (b * 32 >= mine) break;
-                            uint32_t v[32];
-                            tmem_ld32(tSh + 32u * b, v);
-                            tmem_wait_ld();
-                            float mx[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
-#pragma unroll
-                            for (int e = 0; e < 32; ++e)
-                                if (b * 32 + e < mine) mx[e & 3] = fmaxf(mx[e & 3], __uint_as_float(v[e]));
-                            tmax = fmaxf(tmax, fmaxf(fmaxf(mx[0], mx[1]), fmaxf(mx[2], mx[3])));
-                        }
-                        float t0, t1;
-                        pair_xch(tmax, t0, t1);
-                        const float tm2 = fmaxf(t0, t1) * p.c2;
-                        if (j == 0) {
-                            m_ref = tm2;                  // l = 0, O not started
-                        } else {
-                            const bool need = tm2 > m_ref + kRescaleThreshold;
-                            if (__any_sync(0xffffffffu, need)) {
-                                const float up = need ? ceilf(tm2 - m_ref) : 0.f;
-                                const float f = ex2_approx(-up);              // exact power of two (1 for rows that are fine)
-                                l *= f;
-                                // PV(s, j-1) completed before S(s, j) was committed: O is at rest
-#pragma unroll 1
-                                for (int ch = 0; ch < kOHalf / 32; ++ch) {
-                                    uint32_t o[32];
-                                    tmem_ld32(tOh + 32u * ch, o);
-                                    tmem_wait_ld();
-#pragma unroll
-                                    for (int e = 0; e < 32; ++e) o[e] = __float_as_uint(__uint_as_float(o[e]) * f);
-                                    tmem_st32(tOh + 32u * ch, o);
-                                }
-                                m_ref += up;
-                            }
-                        }
-                        uint32_t w[2][16];
-#pragma unroll
-                        for (int b = 0; b < 2; ++b) {
-#pragma unroll
-                            for (int e = 0; e < 16; ++e) w[b][e] = 0u;
-                            if (b * 32 < mine) {
-                                uint32_t v[32];
-                                tmem_ld32(tSh + 32u * b, v);
-                                tmem_wait_ld();
-                                float ls[4] = {0.f, 0.f, 0.f, 0.f};
-#pragma unroll
-                                for (int e = 0; e < 32; e += 2) {
-                                    float p0 = ex2_approx(fmaf(__uint_as_float(v[e]), p.c2, -m_ref));
-                                    float p1 = ex2_approx(fmaf(__uint_as_float(v[e + 1]), p.c2, -m_ref));
-                                    if (b * 32 + e >= mine) p0 = 0.f;
-                                    if (b * 32 + e + 1 >= mine) p1 = 0.f;
-                                    ls[(e >> 1) & 3] += p0 + p1;
-                                    w[b][e >> 1] = pack_bf16x2(p0, p1);
-                                }
-                                l += (ls[0] + ls[1]) + (ls[2] + ls[3]);
-                            }
-                        }
-                        tmem_st16(tSh, w[0]);
-                        tmem_st16(tSh + 16u, w[1]);
-                    }
-                    tmem_wait_st();
-                    tc_fence_before();
-                    mbar_arrive(bar(BAR_PREADY0 + s));
-                    if (row == 0) PDLLM_TR(33, 2 * j + s);
-                    if (s) {
-                        m1 = m_ref;
-                        l1 = l;
-                    } else {
-                        m0 = m_ref;
-                        l0 = l;
+                        tmem_st32(tS, *reinterpret_cast<uint32_t(*)[32]>(w));
+                        tmem_st32(tS + 32u, *reinterpret_cast<uint32_t(*)[32]>(w + 32));
+                        l += lsum;
+                        // 2^pend >= lsum >= the row's largest P: after the raise the same logits give P <= 1
+                        if (lsum > kSoftLimit) pend = (float)(((__float_as_int(lsum) >> 23) & 0xff) - 126);
                     }
                 }
+                if (careful) {
+                    // Ragged tail tile (possibly the stream's first) or a row sum beyond 2^kHardOctaves: row max over the
+                    // valid columns -> reference (raised by whole octaves once it exists, so that l and O rescale exactly)
+                    // -> masked exponentials -> P.  Nothing of this tile has been stored yet: S is read twice.
+                    const int nblk = (n_valid + 31) >> 5;
+                    float tmax = -INFINITY;
+#pragma unroll 1
+                    for (int b = 0; b < nblk; ++b) {
+                        uint32_t v[32];
+                        tmem_ld32(tS + 32u * b, v);
+                        tmem_wait_ld();
+                        float mx[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
+#pragma unroll
+                        for (int e = 0; e < 32; ++e)
+                            if (b * 32 + e < n_valid) mx[e & 3] = fmaxf(mx[e & 3], __uint_as_float(v[e]));
+                        tmax = fmaxf(tmax, fmaxf(fmaxf(mx[0], mx[1]), fmaxf(mx[2], mx[3])));
+                    }
+                    const float tm2 = tmax * p.c2;
+                    if (j == 0) {
+                        m_ref = tm2;                      // l = 0, O not started
+                    } else {
+                        const bool need = tm2 > m_ref + kRescaleThreshold;
+                        if (__any_sync(0xffffffffu, need)) {
+                            const float up = need ? ceilf(tm2 - m_ref) : 0.f;
+                            const float f = ex2_approx(-up);
+                            l *= f;
+                            scale_O(f);
+                            m_ref += up;
+                        }
+                    }
+#pragma unroll 1
+                    for (int b = 0; b < 4; ++b) {
+                        uint32_t w[16];
+#pragma unroll
+                        for (int e = 0; e < 16; ++e) w[e] = 0u;
+                        if (b < nblk) {
+                            uint32_t v[32];
+                            tmem_ld32(tS + 32u * b, v);
+                            tmem_wait_ld();
+                            float ls[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+                            for (int e = 0; e < 32; e += 2) {
+                                float p0 = ex2_approx(fmaf(__uint_as_float(v[e]), p.c2, -m_ref));
+                                float p1 = ex2_approx(fmaf(__uint_as_float(v[e + 1]), p.c2, -m_ref));
+                                if (b * 32 + e >= n_valid) p0 = 0.f;
+                                if (b * 32 + e + 1 >= n_valid) p1 = 0.f;
+                                ls[(e >> 1) & 3] += p0 + p1;
+                                w[e >> 1] = pack_bf16x2(p0, p1);
+                            }
+                            l += (ls[0] + ls[1]) + (ls[2] + ls[3]);
+                        }
+                        // P block b (16 packed columns) must not overwrite S columns that are still to be read: block b of
+                        // P lands on S columns 16b..16b+15 <= 32b, already consumed
+                        tmem_st16(tS + 16u * b, w);
+                    }
+                }
+                tmem_wait_st();
+                tc_fence_before();
+                mbar_arrive(bar(BAR_PREADY0 + s));
             }
-            if (row == 0) PDLLM_TR(34, ns0);
             // ------------------------------- epilogue -------------------------------
             // Pair items: one output tile per stream.  Single items (a5 inside the CTA): both streams hold partial
-            // results of the SAME rows, merged here out of TMEM -- every thread already has both (m, l) pairs.
-            const bool merge_other = !it.modeA && it.nt > 1;      // stream 1 had tiles (uniform per item)
-            const bool o_align32 = (reinterpret_cast<uintptr_t>(p.O) & 31u) == 0;
-            const int n_out = it.modeA ? 2 : 1;
-            // whole-row sums (both halves), exchanged while the last P*V are still running
-            float lr0, lr1 = 0.f;
-            {
-                float x0, x1;
-                pair_xch(l0, x0, x1);
-                lr0 = x0 + x1;
-                if (it.modeA || merge_other) {
-                    pair_xch(l1, x0, x1);
-                    lr1 = x0 + x1;
+            // results of the SAME rows; stream 1 publishes its (m, l), stream 0 merges both accumulators out of TMEM.
+            if (pend > 0.f) {                             // a raise still owed: fold it into the statistics only (O is
+                m_ref += pend;                            // normalised by l below, the common factor cancels) ...
+                l *= ex2_approx(-pend);
+            }
+            const float o_fix = pend > 0.f ? ex2_approx(-pend) : 1.f;      // ... but keep O and l on one scale
+            const int qt = it.modeA ? it.q0 + s : it.q0;
+            const int qr = qt * kTileM + row;
+            const bool row_ok = qr < p.rows_g;
+            const int64_t grow = (int64_t)it.bg * p.rows_g + qr;
+            if (n_mine > 0) {
+                mbar_wait(bar(BAR_OREADY0 + s), n_oready++ & 1u);
+                tc_fence_after();
+            }
+            float a_self = o_fix, a_other = 0.f, l_tot = l, m_tot = m_ref;
+            const bool merge_other = !it.modeA && it.nt > 1;    // stream 1 had tiles (uniform per item)
+            if (!it.modeA) {
+                if (s == 1) {
+                    // stream 0 has read the previous single item's values (named barrier 3: it arrives, we wait)
+                    if (n_modeB > 0) asm volatile("bar.sync 3, 256;" ::: "memory");
+                    s_ml[row][0] = m_ref;
+                    s_ml[row][1] = l;
+                    s_ml[row][2] = o_fix;
+                }
+                ++n_modeB;
+                tc_fence_before();
+                asm volatile("bar.sync 2, 256;" ::: "memory");
+                tc_fence_after();
+                if (s == 0) {
+                    const float m1 = s_ml[row][0], l1 = s_ml[row][1], fix1 = s_ml[row][2];
+                    asm volatile("bar.arrive 3, 256;" ::: "memory");
+                    if (merge_other) {
+                        m_tot = fmaxf(m_ref, m1);
+                        const float e0 = ex2_approx(m_ref - m_tot), e1 = ex2_approx(m1 - m_tot);
+                        l_tot = l * e0 + l1 * e1;
+                        a_self = o_fix * e0;
+                        a_other = fix1 * e1;
+                    }
                 }
             }
-#pragma unroll 1
-            for (int s = 0; s < n_out; ++s) {
-                const int qr = (it.q0 + s) * kTileM + row;
-                const bool row_ok = qr < p.rows_g;
-                const int64_t grow = (int64_t)it.bg * p.rows_g + qr;
-                float a_self = 1.f, a_other = 0.f, l_tot = s ? lr1 : lr0, m_tot = s ? m1 : m0;
-                if (merge_other) {
-                    m_tot = fmaxf(m0, m1);
-                    a_self = ex2_approx(m0 - m_tot);
-                    a_other = ex2_approx(m1 - m_tot);
-                    l_tot = lr0 * a_self + lr1 * a_other;
-                }
+            if (it.modeA || s == 0) {
                 const float inv = 1.f / l_tot;
                 const float lse = (m_tot + lg2_approx(l_tot)) * 0.6931471805599453f;
                 const float w_self = a_self * inv, w_other = a_other * inv;
-                const uint32_t tOh = tmem + kOCol + 128u * s + lane_base + (uint32_t)(kOHalf * half);
-                const uint32_t tO_other = tmem + kOCol + 128u + lane_base + (uint32_t)(kOHalf * half);    // stream 1, same rows
-                if (half == 0 && row_ok) {
+                const uint32_t tO_other = tmem + kOCol + 128u + lane_base;    // stream 1's accumulator, same rows
+                const bool o_align32 = (reinterpret_cast<uintptr_t>(p.O) & 31u) == 0;
+                if (row_ok) {
                     if (p.n_splits == 1) p.LSE[grow] = lse;
                     else p.lse_part[(int64_t)it.split * p.total_rows + grow] = lse;
                 }
-                mbar_wait(bar(BAR_OREADY0 + s), (ph_o >> s) & 1u);
-                ph_o ^= 1u << s;
-                if (merge_other) {
-                    mbar_wait(bar(BAR_OREADY1), (ph_o >> 1) & 1u);
-                    ph_o ^= 2u;
-                }
-                tc_fence_after();
-                if (row == 0) PDLLM_TR(37, s);
-                constexpr int kCh = kOHalf / 32;          // 32-column chunks of this thread's O columns (1 or 2)
-                uint32_t oa[32], ob[32];
-                tmem_ld32(tOh, oa);
-                if (kCh == 2) tmem_ld32(tOh + 32u, ob);
-                tmem_wait_ld();
-                if (row == 0) PDLLM_TR(38, s);
-                auto emit = [&](uint32_t(&o)[32], int ch) {
+#pragma unroll 1
+                for (int ch = 0; ch < D / 32; ++ch) {
+                    uint32_t o[32];
+                    tmem_ld32(tO + 32u * ch, o);
+                    tmem_wait_ld();
                     float f[32];
 #pragma unroll
                     for (int e = 0; e < 32; ++e) f[e] = __uint_as_float(o[e]) * w_self;
@@ -757,13 +702,18 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
 #pragma unroll
                         for (int e = 0; e < 32; ++e) f[e] = fmaf(__uint_as_float(o[e]), w_other, f[e]);
                     }
+                    if (ch == D / 32 - 1) {
+                        // the accumulator(s) are in registers: hand them back before the last stores
+                        tc_fence_before();
+                        mbar_arrive(bar(BAR_OFREE0 + s));
+                        if (merge_other) mbar_arrive(bar(BAR_OFREE1));      // stream 0 has drained stream 1's accumulator
+                    }
                     if (row_ok) {
-                        const int col0 = kOHalf * half + ch * 32;
                         if (p.n_splits == 1) {
                             uint32_t u[16];
 #pragma unroll
                             for (int e = 0; e < 16; ++e) u[e] = pack_bf16x2(f[2 * e], f[2 * e + 1]);
-                            uint16_t *dst = p.O + grow * D + col0;
+                            uint16_t *dst = p.O + grow * D + ch * 32;
                             if (o_align32) {              // whole 32-byte sectors per lane (rows are 2*D bytes apart)
                                 st_global_v8(dst, u[0], u[1], u[2], u[3], u[4], u[5], u[6], u[7]);
                                 st_global_v8(dst + 16, u[8], u[9], u[10], u[11], u[12], u[13], u[14], u[15]);
@@ -774,31 +724,17 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
                             }
                         } else {
                             float4 *dst =
-                                reinterpret_cast<float4 *>(p.O_part + ((int64_t)it.split * p.total_rows + grow) * D + col0);
+                                reinterpret_cast<float4 *>(p.O_part + ((int64_t)it.split * p.total_rows + grow) * D + ch * 32);
 #pragma unroll
                             for (int q4 = 0; q4 < 8; ++q4)
                                 dst[q4] = make_float4(f[q4 * 4 + 0], f[q4 * 4 + 1], f[q4 * 4 + 2], f[q4 * 4 + 3]);
                         }
                     }
-                };
-                if (merge_other) {
-                    // stream 1's chunk comes through the same registers: one chunk at a time
-                    emit(oa, 0);
-                    if (kCh == 2) emit(ob, 1);
-                    tc_fence_before();
-                    mbar_arrive(bar(BAR_OFREE0));
-                    mbar_arrive(bar(BAR_OFREE1));         // stream 1's accumulator has been drained too
-                } else {
-                    // the accumulator is in registers: hand it back before the stores
-                    tc_fence_before();
-                    mbar_arrive(bar(BAR_OFREE0 + s));
-                    emit(oa, 0);
-                    if (kCh == 2) emit(ob, 1);
                 }
-                if (row == 0) PDLLM_TR(39, s);
             }
-            if (row == 0) PDLLM_TR(35, ns0);
         }
+    } else {
+        setmaxnreg_dec<kOtherRegs>();                     // warps 13-15 of the MMA warp's group: nothing to do
     }
     tc_fence_before();
     __syncthreads();

@@ -1,21 +1,26 @@
 // pdllm_api.cu -- the C-ABI entry points of include/pdllm.h: host-side validation, shape
 // resolution, split-count choice, workspace carving and the enqueue sequences.  No arithmetic
 // of the method happens on the host.
+#include <atomic>
 #include <cmath>
 #include <cstdint>
+#include <cstdlib>
+#include <cstring>
 
 #include "pdllm_internal.h"
 
 namespace pdllm {
 
+// SM count of the CURRENT device (an immutable hardware fact, remembered per device index after the first query).
 int device_num_sms() {
-    static int sms = [] {
-        int dev = 0, n = 0;
-        if (cudaGetDevice(&dev) != cudaSuccess) return 148;
-        if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) return 148;
-        return n;
-    }();
-    return sms;
+    constexpr int kMaxDev = 64;
+    static std::atomic<int> cache[kMaxDev];
+    int dev = 0, n = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return 148;
+    if (dev >= 0 && dev < kMaxDev && (n = cache[dev].load(std::memory_order_relaxed)) > 0) return n;
+    if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) return 148;
+    if (dev >= 0 && dev < kMaxDev) cache[dev].store(n, std::memory_order_relaxed);
+    return n;
 }
 
 namespace {
@@ -76,7 +81,7 @@ double split_cost_us(const Dims &d, int S, int sms) {
 }
 
 int auto_splits(const Dims &d, int num_sms) {
-    const int sms = num_sms > 0 ? num_sms : 148;
+    const int sms = num_sms > 0 ? num_sms : device_num_sms();
     const int T = kv_tiles(d);
     const int Smax = T < 64 ? T : 64;
     int best = 1;
@@ -128,6 +133,24 @@ HostScratch host_scratch(const Dims &d, int S) {
 
 int cuda_rc(cudaError_t e) { return e == cudaSuccess ? PDLLM_OK : PDLLM_ERR_CUDA; }
 
+// PDLLM_DEBUG_VALIDATE=1 (include/pdllm.h, "DEBUG SWITCH"): check the index lists on the device, synchronise, report.
+bool debug_validate_on() {
+    const char *e = std::getenv("PDLLM_DEBUG_VALIDATE");
+    return e && e[0] != '\0' && std::strcmp(e, "0") != 0;
+}
+int debug_validate(const Dims &d, const int32_t *chunk_ids, const int32_t *keep, cudaStream_t st) {
+    if (!debug_validate_on() || (!chunk_ids && !keep)) return PDLLM_OK;
+    int32_t *flag = nullptr, h = 0;
+    if (cudaMalloc(&flag, sizeof(int32_t)) != cudaSuccess) return PDLLM_ERR_CUDA;
+    cudaError_t e = cudaMemsetAsync(flag, 0, sizeof(int32_t), st);
+    if (e == cudaSuccess) e = launch_validate(d, chunk_ids, keep, flag, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(&h, flag, sizeof(int32_t), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    cudaFree(flag);
+    if (e != cudaSuccess) return PDLLM_ERR_CUDA;
+    return h ? PDLLM_ERR_DATA : PDLLM_OK;
+}
+
 }  // namespace
 }  // namespace pdllm
 
@@ -146,6 +169,7 @@ const char *pdllm_strerror(int status) {
         case PDLLM_ERR_WORKSPACE: return "workspace too small";
         case PDLLM_ERR_UNSUPPORTED: return "unsupported request";
         case PDLLM_ERR_CUDA: return "CUDA call or launch failed";
+        case PDLLM_ERR_DATA: return "PDLLM_DEBUG_VALIDATE: a chunk id or token-keep list on the device is malformed";
         default: return "unknown pdllm status";
     }
 }
@@ -195,6 +219,7 @@ int pdllm_gather_idx(const pdllm_shape *shape, const int32_t *chunk_ids, const i
     if (!shape || !chunk_ids || !gather_idx) return PDLLM_ERR_NULL;
     Dims d;
     if (int rc = resolve(shape, token_keep_idx != nullptr, &d)) return rc;
+    if (int rc = debug_validate(d, chunk_ids, token_keep_idx, static_cast<cudaStream_t>(stream))) return rc;
     return cuda_rc(launch_gather_idx(d, chunk_ids, token_keep_idx, gather_idx, static_cast<cudaStream_t>(stream)));
 }
 
@@ -238,26 +263,6 @@ int attn_impl(const Dims &d, const void *Q_dec, const void *Kcache, const void *
     return record(ev_end, st);
 }
 
-// The side stream of pdllm_step_host (one per host thread and device, created on first use, kept for the process).
-struct SideStream {
-    cudaStream_t stream = nullptr;
-    cudaEvent_t fork = nullptr, join = nullptr;
-    int device = -1;
-};
-SideStream *side_stream() {
-    static thread_local SideStream ss[16];
-    int dev = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 16) return nullptr;
-    SideStream &s = ss[dev];
-    if (s.device != dev) {
-        if (cudaStreamCreateWithFlags(&s.stream, cudaStreamNonBlocking) != cudaSuccess) return nullptr;
-        if (cudaEventCreateWithFlags(&s.fork, cudaEventDisableTiming) != cudaSuccess) return nullptr;
-        if (cudaEventCreateWithFlags(&s.join, cudaEventDisableTiming) != cudaSuccess) return nullptr;
-        s.device = dev;
-    }
-    return &s;
-}
-
 int attn_validate(const pdllm_shape *shape, const void *Q_dec, const void *Kcache, const void *Vcache,
                   const int32_t *chunk_ids, const int32_t *token_keep_idx, const void *K_dec, const void *V_dec,
                   int32_t n_splits, void *O, float *LSE, void *workspace, size_t workspace_bytes, Dims *d, int *S) {
@@ -268,8 +273,12 @@ int attn_validate(const pdllm_shape *shape, const void *Q_dec, const void *Kcach
         !aligned16(O) || !aligned16(workspace))
         return PDLLM_ERR_ALIGN;
     *S = effective_splits(*d, n_splits, device_num_sms());
-    const size_t need = workspace_for(*d, *S);
-    if (!workspace || workspace_bytes < need) return PDLLM_ERR_WORKSPACE;
+    if (!workspace) return PDLLM_ERR_WORKSPACE;
+    // n_splits == 0 leaves the count to the library: should the caller have sized the workspace for another SM count
+    // (pdllm_workspace_bytes with a num_sms that is not this device's), the largest count that fits is taken
+    if (n_splits == 0)
+        while (*S > 1 && workspace_bytes < workspace_for(*d, *S)) --*S;
+    if (workspace_bytes < workspace_for(*d, *S)) return PDLLM_ERR_WORKSPACE;
     return PDLLM_OK;
 }
 
@@ -284,6 +293,7 @@ int pdllm_sparse_attn(const pdllm_shape *shape, const void *Q_dec, const void *K
     if (int rc = attn_validate(shape, Q_dec, Kcache, Vcache, chunk_ids, token_keep_idx, K_dec, V_dec, n_splits, O, LSE,
                                workspace, workspace_bytes, &d, &S))
         return rc;
+    if (int rc = debug_validate(d, chunk_ids, token_keep_idx, static_cast<cudaStream_t>(stream))) return rc;
     return attn_impl(d, Q_dec, Kcache, Vcache, chunk_ids, token_keep_idx, K_dec, V_dec, S, O, LSE, gather_idx_out,
                      workspace, false, nullptr, nullptr, static_cast<cudaStream_t>(stream));
 }
@@ -302,6 +312,7 @@ int pdllm_step_profiled(const pdllm_shape *shape, const void *Q_dec, const void 
         return rc;
     if (!aligned16(scores_out)) return PDLLM_ERR_ALIGN;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (int rc = debug_validate(d, nullptr, token_keep_idx, st)) return rc;
     // the attention's work-item counter is cleared here, far ahead of its kernel (off the step's critical path)
     if (int rc = cuda_rc(cudaMemsetAsync(workspace, 0, sizeof(int32_t), st))) return rc;
     if (int rc = record(ev ? ev->begin : nullptr, st)) return rc;
@@ -325,7 +336,7 @@ int pdllm_step(const pdllm_shape *shape, const void *Q_dec, const void *Kcache, 
 int pdllm_step_host(const pdllm_shape *shape, const void *h_Q_dec, const void *h_K_dec, const void *h_V_dec,
                     const void *d_Kcache, const void *d_Vcache, const int32_t *d_token_keep_idx, int32_t n_splits,
                     void *h_O, float *h_LSE, int32_t *h_chunk_ids, void *d_scratch, size_t scratch_bytes,
-                    pdllm_stream_t stream) {
+                    const pdllm_side_stream *side, pdllm_stream_t stream) {
     if (!shape || !h_Q_dec || !h_K_dec || !h_V_dec || !d_Kcache || !d_Vcache || !h_O || !h_LSE || !h_chunk_ids || !d_scratch)
         return PDLLM_ERR_NULL;
     if (n_splits < 0) return PDLLM_ERR_SHAPE;
@@ -347,22 +358,27 @@ int pdllm_step_host(const pdllm_shape *shape, const void *h_Q_dec, const void *h
                                &dv, &Sv))
         return rc;
     if (shape->L_q > shape->L) return PDLLM_ERR_SHAPE;
-    // Scoring and top-K need only Q: K_dec / V_dec travel on a library-owned side stream underneath them and join
+    if (int rc = debug_validate(dv, nullptr, d_token_keep_idx, st)) return rc;
+    // Scoring and top-K need only Q: with a caller-supplied side stream K_dec / V_dec travel underneath them and join
     // before the attention (fork after everything queued on `stream`, so an earlier step's kernels have let go of
-    // the scratch buffers).
-    SideStream *ss = side_stream();
-    if (!ss) return PDLLM_ERR_CUDA;
-    if (cudaEventRecord(ss->fork, st) != cudaSuccess) return PDLLM_ERR_CUDA;
-    if (cudaStreamWaitEvent(ss->stream, ss->fork, 0) != cudaSuccess) return PDLLM_ERR_CUDA;
+    // the scratch buffers).  Without one, all copies go on `stream` in order.
+    if (side && (!side->stream || !side->ev_fork || !side->ev_join)) return PDLLM_ERR_NULL;
+    cudaStream_t st2 = side ? static_cast<cudaStream_t>(side->stream) : st;
+    cudaEvent_t ev_fork = side ? static_cast<cudaEvent_t>(side->ev_fork) : nullptr;
+    cudaEvent_t ev_join = side ? static_cast<cudaEvent_t>(side->ev_join) : nullptr;
+    if (side) {
+        if (cudaEventRecord(ev_fork, st) != cudaSuccess) return PDLLM_ERR_CUDA;
+        if (cudaStreamWaitEvent(st2, ev_fork, 0) != cudaSuccess) return PDLLM_ERR_CUDA;
+    }
     if (cudaMemcpyAsync(base + h.q, h_Q_dec, qb, cudaMemcpyHostToDevice, st) != cudaSuccess) return PDLLM_ERR_CUDA;
-    if (cudaMemcpyAsync(base + h.kd, h_K_dec, kb, cudaMemcpyHostToDevice, ss->stream) != cudaSuccess) return PDLLM_ERR_CUDA;
-    if (cudaMemcpyAsync(base + h.vd, h_V_dec, kb, cudaMemcpyHostToDevice, ss->stream) != cudaSuccess) return PDLLM_ERR_CUDA;
-    if (cudaEventRecord(ss->join, ss->stream) != cudaSuccess) return PDLLM_ERR_CUDA;
+    if (cudaMemcpyAsync(base + h.kd, h_K_dec, kb, cudaMemcpyHostToDevice, st2) != cudaSuccess) return PDLLM_ERR_CUDA;
+    if (cudaMemcpyAsync(base + h.vd, h_V_dec, kb, cudaMemcpyHostToDevice, st2) != cudaSuccess) return PDLLM_ERR_CUDA;
+    if (side && cudaEventRecord(ev_join, st2) != cudaSuccess) return PDLLM_ERR_CUDA;
     if (int rc = cuda_rc(cudaMemsetAsync(base + h.ws, 0, sizeof(int32_t), st))) return rc;
     if (int rc = cuda_rc(launch_score(dv, base + h.q, (int64_t)dv.H * dv.L * dv.d, (int64_t)dv.L * dv.d, d_Kcache, scores, st)))
         return rc;
     if (int rc = cuda_rc(launch_topk(dv, scores, ids, st))) return rc;
-    if (cudaStreamWaitEvent(st, ss->join, 0) != cudaSuccess) return PDLLM_ERR_CUDA;
+    if (side && cudaStreamWaitEvent(st, ev_join, 0) != cudaSuccess) return PDLLM_ERR_CUDA;
     if (int rc = attn_impl(dv, base + h.q, d_Kcache, d_Vcache, ids, d_token_keep_idx, base + h.kd, base + h.vd, Sv,
                            base + h.o, reinterpret_cast<float *>(base + h.lse), nullptr, base + h.ws, true, nullptr, nullptr,
                            st))

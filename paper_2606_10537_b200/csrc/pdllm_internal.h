@@ -26,6 +26,8 @@ cudaError_t launch_topk(const Dims &s, const float *scores, int32_t *chunk_ids, 
 // ---- a3
 cudaError_t launch_gather_idx(const Dims &s, const int32_t *chunk_ids, const int32_t *keep, int32_t *gather_idx,
                               cudaStream_t st);
+// ---- PDLLM_DEBUG_VALIDATE: *flag |= bits for malformed chunk_ids [B,H_kv,K] / keep [B,H_kv,N,Bk] (either may be NULL)
+cudaError_t launch_validate(const Dims &s, const int32_t *chunk_ids, const int32_t *keep, int32_t *flag, cudaStream_t st);
 // ---- a5
 cudaError_t launch_combine(const float *O_part, const float *lse_part, int S, int64_t rows, int d, void *O, float *LSE,
                            cudaStream_t st);

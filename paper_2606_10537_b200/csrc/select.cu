@@ -97,7 +97,35 @@ __global__ void gather_idx_kernel(const int32_t *__restrict__ ids, const int32_t
     out[i] = n * Cp + slot;
 }
 
+// PDLLM_DEBUG_VALIDATE (include/pdllm.h): bit 0 = a chunk id outside [0, N); bit 1 = keep[..,0] != 0 (the BOS slot, R7);
+// bit 2 = a keep slot outside [0, C]; bit 3 = a keep list that is not strictly ascending.
+__global__ void validate_kernel(const int32_t *__restrict__ ids, int64_t n_ids, int N, const int32_t *__restrict__ keep,
+                                int64_t n_keep, int Bk, int C, int32_t *flag) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    int bad = 0;
+    if (ids && i < n_ids) {
+        const int n = ids[i];
+        if (n < 0 || n >= N) bad |= 1;
+    }
+    if (keep && i < n_keep) {
+        const int t = (int)(i % Bk), v = keep[i];
+        if (t == 0 && v != 0) bad |= 2;
+        if (v < 0 || v > C) bad |= 4;
+        if (t > 0 && keep[i - 1] >= v) bad |= 8;
+    }
+    if (bad) atomicOr(flag, bad);
+}
+
 }  // namespace
+
+cudaError_t launch_validate(const Dims &s, const int32_t *chunk_ids, const int32_t *keep, int32_t *flag, cudaStream_t st) {
+    const int64_t n_ids = chunk_ids ? (int64_t)s.B * s.H_kv * s.K : 0;
+    const int64_t n_keep = keep ? (int64_t)s.B * s.H_kv * s.N * s.Bk : 0;
+    const int64_t total = n_ids > n_keep ? n_ids : n_keep;
+    if (total == 0) return cudaSuccess;
+    validate_kernel<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(chunk_ids, n_ids, s.N, keep, n_keep, s.Bk, s.C, flag);
+    return cudaGetLastError();
+}
 
 cudaError_t launch_topk(const Dims &s, const float *scores, int32_t *chunk_ids, cudaStream_t st) {
     const int rows = s.B * s.H_kv;

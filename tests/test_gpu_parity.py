@@ -219,8 +219,14 @@ def test_step_host_matches_step(B):
     hL = torch.empty((w.B, w.H, w.L), dtype=torch.float32).pin_memory()
     hI = torch.empty((w.B, w.H_kv, w.K), dtype=torch.int32).pin_memory()
     scratch = torch.empty((B.step_host_scratch_bytes(shape, 2, B.num_sms()),), dtype=torch.uint8, device="cuda")
-    B.step_host(shape, hQ, hK, hV, dev["Kcache"], dev["Vcache"], dev["keep"], 2, hO, hL, hI, scratch)
+    B.step_host(shape, hQ, hK, hV, dev["Kcache"], dev["Vcache"], dev["keep"], 2, hO, hL, hI, scratch)      # one stream
     torch.cuda.synchronize()
+    hO2, hL2, hI2 = torch.empty_like(hO).pin_memory(), torch.empty_like(hL).pin_memory(), torch.empty_like(hI).pin_memory()
+    side = B.SideStream()
+    for _ in range(3):                               # with the caller's side stream, back to back on one scratch
+        B.step_host(shape, hQ, hK, hV, dev["Kcache"], dev["Vcache"], dev["keep"], 2, hO2, hL2, hI2, scratch, side=side)
+    torch.cuda.synchronize()
+    assert torch.equal(hO.view(torch.int16), hO2.view(torch.int16)) and torch.equal(hL, hL2) and torch.equal(hI, hI2)
     out = B.step(shape, dev["Q_dec"], dev["Kcache"], dev["Vcache"], dev["keep"], dev["K_dec"], dev["V_dec"], n_splits=2)
     torch.cuda.synchronize()
     assert torch.equal(hO.view(torch.int16), out["O"].cpu().view(torch.int16))
@@ -239,6 +245,41 @@ def test_errors(B):
     with pytest.raises(B.PdllmError):                                             # workspace too small for 2 splits
         B.sparse_attn(shape, dev["Q_dec"], dev["Kcache"], dev["Vcache"], dev_i32(inp["planted"]), dev["keep"],
                       dev["K_dec"], dev["V_dec"], n_splits=2, workspace=ws)
+
+
+def test_debug_validate_switch(B, monkeypatch):
+    """PDLLM_DEBUG_VALIDATE=1 (include/pdllm.h "DEBUG SWITCH"): malformed chunk ids / keep lists are reported as
+    PDLLM_ERR_DATA (-7) with nothing enqueued; well-formed lists pass and give the usual result."""
+    w, inp = _inputs("tiny")
+    dev = to_device(inp)
+    shape = B.Shape.of(w)
+    ids = dev_i32(inp["planted"])
+    monkeypatch.setenv("PDLLM_DEBUG_VALIDATE", "1")
+    O_ref, LSE_ref = oracle.attn(inp["Q_dec"], inp["Kcache"], inp["Vcache"], inp["planted"], inp["keep"], inp["K_dec"], inp["V_dec"])
+    O, LSE = B.sparse_attn(shape, dev["Q_dec"], dev["Kcache"], dev["Vcache"], ids, dev["keep"], dev["K_dec"], dev["V_dec"], n_splits=1)
+    torch.cuda.synchronize()
+    check_O(O, O_ref)
+
+    def expect_data_error(fn):
+        with pytest.raises(B.PdllmError, match="-7"):
+            fn()
+
+    attn = lambda i, k: B.sparse_attn(shape, dev["Q_dec"], dev["Kcache"], dev["Vcache"], i, k, dev["K_dec"], dev["V_dec"], n_splits=1)
+    bad_ids = ids.clone(); bad_ids[0, 1, 0] = w.N                      # chunk id == N
+    expect_data_error(lambda: attn(bad_ids, dev["keep"]))
+    bad_ids = ids.clone(); bad_ids[0, 0, 1] = -1
+    expect_data_error(lambda: B.gather_idx(shape, bad_ids, dev["keep"]))
+    k = dev["keep"].clone(); k[0, 2, 3, 0] = 1                         # BOS slot not kept first
+    expect_data_error(lambda: attn(ids, k))
+    k = dev["keep"].clone(); k[0, 1, 5, w.Bk - 1] = w.C + 1            # slot beyond the chunk
+    expect_data_error(lambda: attn(ids, k))
+    k = dev["keep"].clone(); k[0, 3, 7, 5] = k[0, 3, 7, 4]             # not strictly ascending
+    expect_data_error(lambda: attn(ids, k))
+    expect_data_error(lambda: B.step(shape, dev["Q_dec"], dev["Kcache"], dev["Vcache"], k, dev["K_dec"], dev["V_dec"], n_splits=1))
+    monkeypatch.setenv("PDLLM_DEBUG_VALIDATE", "0")                    # switch off: the well-formed call is untouched
+    O2, _ = attn(ids, dev["keep"])
+    torch.cuda.synchronize()
+    assert torch.equal(O2.view(torch.int16), O.view(torch.int16))
 
 
 # --------------------------------------------------------------------------- rare paths of the single-pass softmaxes

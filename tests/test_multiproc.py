@@ -63,3 +63,11 @@ def test_reference_arm_runs_on_rank0_only():
     line = json.loads(res.stdout.strip().splitlines()[-1])
     assert line["impl"] == "reference" and line["cpu_baseline"]["kind"] == "oracle" and line["value"] > 0
     assert line["e2e"]["h2d_bytes_per_step"] == 0 and line["unit"] == "us"
+
+
+def test_gpus_flag_without_one_rank_per_gpu_is_refused():
+    """`bench.py --gpus 2` outside torchrun must not print an n_gpus=1 line: it exits non-zero (replicas need one rank per GPU)."""
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK")}
+    res = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--steps", "1", "--warmup", "0",
+                          "--workload", "tiny"], capture_output=True, text=True, env=env, timeout=300)
+    assert res.returncode != 0 and res.stdout.strip() == "" and "one rank per GPU" in res.stderr
