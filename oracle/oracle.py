@@ -18,14 +18,15 @@ import numpy as np
 
 _HERE = Path(__file__).resolve().parent
 _SRC = _HERE / "pdllm_oracle.c"
+_SRC_NEXT = _HERE / "pdllm_oracle_next.c"      # the rows after the hot path
 _LIB = _HERE / "libpdllm_oracle.so"
 _lib = None
 
 
 def build(force: bool = False) -> Path:
     """Compile the oracle with gcc (-O2, OpenMP over (b,h) only; no SIMD intrinsics, no tuning)."""
-    if force or not _LIB.exists() or _LIB.stat().st_mtime < _SRC.stat().st_mtime:
-        cmd = ["gcc", "-O2", "-std=c11", "-fopenmp", "-fPIC", "-shared", str(_SRC), "-o", str(_LIB), "-lm"]
+    if force or not _LIB.exists() or _LIB.stat().st_mtime < max(_SRC.stat().st_mtime, _SRC_NEXT.stat().st_mtime):
+        cmd = ["gcc", "-O2", "-std=c11", "-fopenmp", "-fPIC", "-shared", str(_SRC), str(_SRC_NEXT), "-o", str(_LIB), "-lm"]
         subprocess.run(cmd, check=True)
     return _LIB
 
@@ -148,6 +149,87 @@ def step(Q_dec, Kcache, Vcache, keep, K_dec, V_dec, K, L_q, scale=None, head_mas
     gi = gather_idx(ids, keep, N, Cp - 1)
     O, LSE = attn(Q_dec, Kcache, Vcache, ids, keep, K_dec, V_dec, scale, head_mask=head_mask)
     return dict(scores=sc, ids=ids, gather_idx=gi, O=O, LSE=LSE)
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# rows after the hot path; pdllm_oracle_next.c
+def token_scores(Q, Kcache, L_q, scale=None):
+    """NEXT-1 (Eq. 5, query->chunk term; R22).  -> e f64 [B,H_kv,N,C+1], each chunk's slots summing to G*L_q."""
+    Q = _u16(Q); Kcache = _u16(Kcache)
+    B, H, Lr, d = Q.shape
+    _, H_kv, N, Cp, _ = Kcache.shape
+    scale = 1.0 / np.sqrt(d) if scale is None else scale
+    e = np.empty((B, H_kv, N, Cp), np.float64)
+    rc = _load().oracle_token_scores(_p(Q, ctypes.c_uint16), ctypes.c_int64(H * Lr * d), ctypes.c_int64(Lr * d),
+                                     _p(Kcache, ctypes.c_uint16), B, H, H_kv, d, N, Cp - 1, L_q, ctypes.c_double(scale),
+                                     _p(e, ctypes.c_double))
+    assert rc == 0, rc
+    return e
+
+
+def topb(e, Bk):
+    """NEXT-1 (R7).  e [..., C+1] (any float dtype, widened exactly) -> keep int32 [..., Bk]: slot 0 + the
+    Bk-1 best of slots 1..C, ties to the lower slot, ascending."""
+    e = np.ascontiguousarray(e, dtype=np.float64)
+    Cp = e.shape[-1]
+    keep = np.empty(e.shape[:-1] + (Bk,), np.int32)
+    rc = _load().oracle_topb(_p(e, ctypes.c_double), ctypes.c_int64(e.size // Cp), Cp - 1, Bk, _p(keep, ctypes.c_int32))
+    assert rc == 0, rc
+    return keep
+
+
+def prefill_attn(Q, K, V, scale=None):
+    """NEXT-2 (Eq. 2).  Q uint16 [S,H,T,d], K,V uint16 [S,H_kv,T,d] -> O f64 [S,H,T,d], LSE f64 [S,H,T]."""
+    Q = _u16(Q); K = _u16(K); V = _u16(V)
+    S, H, T, d = Q.shape
+    H_kv = K.shape[1]
+    scale = 1.0 / np.sqrt(d) if scale is None else scale
+    O = np.empty((S, H, T, d), np.float64)
+    LSE = np.empty((S, H, T), np.float64)
+    rc = _load().oracle_prefill_attn(_p(Q, ctypes.c_uint16), _p(K, ctypes.c_uint16), _p(V, ctypes.c_uint16), S, H, H_kv, T, d,
+                                     ctypes.c_double(scale), _p(O, ctypes.c_double), _p(LSE, ctypes.c_double))
+    assert rc == 0, rc
+    return O, LSE
+
+
+def compact_kv(Kcache, Vcache, gather_idx_):
+    """NEXT-3.  Kcache,Vcache uint16 [B,H_kv,N,C+1,d]; gather_idx int32 [B,H_kv,S_pre]
+    -> Kc, Vc uint16 [B,H_kv,S_pre,d] (bit copies of the selected rows)."""
+    Kcache = _u16(Kcache); Vcache = _u16(Vcache)
+    gi = np.ascontiguousarray(gather_idx_, dtype=np.int32)
+    B, H_kv, N, Cp, d = Kcache.shape
+    S_pre = gi.shape[-1]
+    Kc = np.empty((B, H_kv, S_pre, d), np.uint16)
+    Vc = np.empty((B, H_kv, S_pre, d), np.uint16)
+    rc = _load().oracle_compact_kv(_p(Kcache, ctypes.c_uint16), _p(Vcache, ctypes.c_uint16), _p(gi, ctypes.c_int32), B, H_kv,
+                                   ctypes.c_int64(N * Cp), S_pre, d, _p(Kc, ctypes.c_uint16), _p(Vc, ctypes.c_uint16))
+    assert rc == 0, rc
+    return Kc, Vc
+
+
+def pooled_keys(Kcache):
+    """NEXT-3 (R23).  -> kbar f64 [B,H_kv,N,d], the mean of each chunk's C+1 cached keys."""
+    Kcache = _u16(Kcache)
+    B, H_kv, N, Cp, d = Kcache.shape
+    kbar = np.empty((B, H_kv, N, d), np.float64)
+    rc = _load().oracle_pooled_keys(_p(Kcache, ctypes.c_uint16), B, H_kv, N, Cp - 1, d, _p(kbar, ctypes.c_double))
+    assert rc == 0, rc
+    return kbar
+
+
+def pooled_scores(Q, kbar, C, L_q, scale=None):
+    """NEXT-3 (R23).  Q uint16 [B,H,Lrows,d]; kbar [B,H_kv,N,d] (widened to f64) -> f64 [B,H_kv,N]."""
+    Q = _u16(Q)
+    kbar = np.ascontiguousarray(kbar, dtype=np.float64)
+    B, H, Lr, d = Q.shape
+    _, H_kv, N, _ = kbar.shape
+    scale = 1.0 / np.sqrt(d) if scale is None else scale
+    out = np.empty((B, H_kv, N), np.float64)
+    rc = _load().oracle_pooled_scores(_p(Q, ctypes.c_uint16), ctypes.c_int64(H * Lr * d), ctypes.c_int64(Lr * d),
+                                      _p(kbar, ctypes.c_double), B, H, H_kv, d, N, C, L_q, ctypes.c_double(scale),
+                                      _p(out, ctypes.c_double))
+    assert rc == 0, rc
+    return out
 
 
 if os.environ.get("PDLLM_ORACLE_BUILD"):

@@ -39,6 +39,8 @@ class Workload:
     alpha: float         # planted key shift, in units of mean(q) (R20)
     unit_logits: bool    # True: Q,K,V ~ N(0,1)/sqrt(d) (config "tiny"); False: N(0,1)
     seed: int
+    token_alpha: float = 0.0   # > 0 (NEXT-1 workloads only): the keys of the slots on the keep list are shifted by
+                               # token_alpha * mean(q) in every chunk, so that top-B token retention has a clear gap
 
     @property
     def G(self): return self.H // self.H_kv
@@ -154,6 +156,8 @@ def make_inputs(w: Workload, threads: int = 8) -> dict:
         b, g = divmod(bg, w.H_kv)
         k = _normal(w.seed, T_KC, bg, (w.N, w.Cp, w.d), sigma)
         k[planted[b, g]] += np.float32(w.alpha) * qbar[b, g]        # shift every row of the planted chunks
+        if w.token_alpha > 0.0 and keep is not None:                  # planted tokens: the kept slots of every chunk
+            k[np.arange(w.N)[:, None], keep[b, g, :, 1:]] += np.float32(w.token_alpha) * qbar[b, g]
         Kc[b, g] = f32_to_bf16_bits(k)
         Vc[b, g] = f32_to_bf16_bits(_normal(w.seed, T_VC, bg, (w.N, w.Cp, w.d), sigma))
 
