@@ -227,6 +227,82 @@ int pdllm_step_host(const pdllm_shape *shape, const void *h_Q_dec, const void *h
                     void *d_scratch, size_t scratch_bytes,
                     const pdllm_side_stream *side, pdllm_stream_t stream);
 
+/* =========================================================================
+ * Rows after the hot path.
+ * ========================================================================= */
+
+/* ---- NEXT-3: the static-selection fast path ---------------
+ * The paper's selection is static: "the retained KV entries of the selected chunks
+ * ... form a static cache that is reused across all T denoising steps";
+ * its FlexAttention kernel reloads that cache every step.  Here the
+ * selected, token-thinned rows are copied ONCE into a contiguous cache, and every
+ * later step runs the same attention kernel over plain 128-row TMA tiles.
+ *
+ * pdllm_compact_kv: row r = k*Bk + t of (b,g) <- cache row
+ * chunk_ids[b,g,k]*(C+1) + token_keep_idx[b,g,chunk_ids[b,g,k],t] (NULL: slot t);
+ * a bit copy of K and V rows.
+ *   Kcompact, Vcompact  device bf16 [B,H_kv,K*Bk,d] (out)                          */
+int pdllm_compact_kv(const pdllm_shape *shape, const void *Kcache, const void *Vcache,
+                     const int32_t *chunk_ids, const int32_t *token_keep_idx,
+                     void *Kcompact, void *Vcompact, pdllm_stream_t stream);
+
+/* Shapes of attention over CONTIGUOUS K/V (no chunk ids, no keep lists): S_pre
+ * prefix rows per KV head followed by L_s decode rows (may be 0).               */
+typedef struct {
+    int32_t B;      /* batch (static cache) or number of independent sequences (prefill), >= 1 */
+    int32_t H;      /* query heads, H % H_kv == 0 */
+    int32_t H_kv;   /* KV heads */
+    int32_t d;      /* head dim, 64 or 128 */
+    int32_t S_pre;  /* contiguous prefix rows per KV head, >= 1 */
+    int32_t L;      /* rows of Q / O / LSE per head, >= 1 */
+    int32_t L_s;    /* rows of K_dec / V_dec per KV head, >= 0 */
+    float   scale;  /* softmax scale; <= 0 selects 1/sqrt(d) */
+} pdllm_dense_shape;
+
+/* a6 for the contiguous kernels; the prefix and the decode rows are tiled separately
+ * (ceil(S_pre/128) + ceil(L_s/128) KV tiles).  Host-only, pure. */
+int32_t pdllm_dense_auto_splits(const pdllm_dense_shape *shape, int32_t num_sms);
+size_t pdllm_dense_workspace_bytes(const pdllm_dense_shape *shape, int32_t n_splits, int32_t num_sms);
+
+/* pdllm_static_attn: a4 + a5 over [ Kcompact/Vcompact rows || K_dec/V_dec rows ]:
+ * exactly pdllm_sparse_attn's result for the chunk ids and keep lists the compact
+ * cache was built from (same keys, same order).
+ *   Q_dec device bf16 [B,H,L,d]; Kcompact,Vcompact device bf16 [B,H_kv,S_pre,d];
+ *   K_dec,V_dec device bf16 [B,H_kv,L_s,d] (NULL allowed when L_s == 0);
+ *   O device bf16 [B,H,L,d] (out); LSE device fp32 [B,H,L] (out);
+ *   workspace >= pdllm_dense_workspace_bytes(shape, n_splits, num_sms) bytes       */
+int pdllm_static_attn(const pdllm_dense_shape *shape, const void *Q_dec, const void *Kcompact,
+                      const void *Vcompact, const void *K_dec, const void *V_dec, int32_t n_splits,
+                      void *O, float *LSE, void *workspace, size_t workspace_bytes,
+                      pdllm_stream_t stream);
+
+/* Pooled-key chunk scorer (R23, ours; parity unpinned by the paper): a cheap
+ * per-step re-selection score that reads N*d instead of N*(C+1)*d per KV head.
+ * pdllm_pool_keys (once, after the prefill):
+ *   kbar[b,g,n,:] = mean over the C+1 cached keys of chunk n (BOS included), fp32.
+ * pdllm_score_chunks_pooled (per step):
+ *   scores[b,g,n] = log(C+1) + scale * < mean of the G*L_q scoring rows, kbar[b,g,n,:] >,
+ * the a1 score with every row of a chunk replaced by the chunk's mean key (by
+ * Jensen's inequality a lower bound of it).  Feed it to pdllm_select_topk.
+ *   kbar device fp32 [B,H_kv,N,d]; Q, strides as in pdllm_score_chunks;
+ *   scores device fp32 [B,H_kv,N] (out)                                            */
+int pdllm_pool_keys(const pdllm_shape *shape, const void *Kcache, float *kbar, pdllm_stream_t stream);
+int pdllm_score_chunks_pooled(const pdllm_shape *shape, const void *Q, int64_t q_batch_stride,
+                              int64_t q_head_stride, const float *kbar, float *scores,
+                              pdllm_stream_t stream);
+
+/* ---- NEXT-2: attention of the chunk prefill (Eq. 2; Fig. 5(a)) --
+ * Each of the shape->B = B*N sequences [BOS; c_i; q; m] (T = S_pre = L rows, L_s = 0)
+ * attends to itself, bidirectionally and unmasked, independently of all
+ * other sequences ("chunks are independent").  Same kernel as
+ * pdllm_static_attn (GQA groups packed into the MMA M dimension, Split-S over the
+ * KV tiles when the sequences alone do not fill the GPU).
+ *   Q device bf16 [B,H,T,d]; K,V device bf16 [B,H_kv,T,d];
+ *   O device bf16 [B,H,T,d] (out); LSE device fp32 [B,H,T] (out)                   */
+int pdllm_prefill_attn(const pdllm_dense_shape *shape, const void *Q, const void *K, const void *V,
+                       int32_t n_splits, void *O, float *LSE, void *workspace,
+                       size_t workspace_bytes, pdllm_stream_t stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -21,12 +21,19 @@ EXPORTS = [
     "pdllm_version", "pdllm_strerror", "pdllm_auto_splits", "pdllm_workspace_bytes",
     "pdllm_step_host_scratch_bytes", "pdllm_score_chunks", "pdllm_select_topk", "pdllm_gather_idx",
     "pdllm_sparse_attn", "pdllm_lse_combine", "pdllm_step", "pdllm_step_profiled", "pdllm_step_host",
+    # rows after the hot path
+    "pdllm_compact_kv", "pdllm_dense_auto_splits", "pdllm_dense_workspace_bytes", "pdllm_static_attn",
+    "pdllm_pool_keys", "pdllm_score_chunks_pooled", "pdllm_prefill_attn",
 ]
 
 
 class PdllmShape(ctypes.Structure):
     _fields_ = [(n, ctypes.c_int32) for n in ("B", "H", "H_kv", "d", "N", "C", "K", "Bk", "L_q", "L", "L_s")] + [
         ("scale", ctypes.c_float)]
+
+
+class PdllmDenseShape(ctypes.Structure):
+    _fields_ = [(n, ctypes.c_int32) for n in ("B", "H", "H_kv", "d", "S_pre", "L", "L_s")] + [("scale", ctypes.c_float)]
 
 
 class PdllmSideStream(ctypes.Structure):
@@ -60,6 +67,27 @@ class Shape:
     def of(w) -> "Shape":
         """From a workloads.Workload."""
         return Shape(w.B, w.H, w.H_kv, w.d, w.N, w.C, w.K, w.Bk, w.L_q, w.L, w.L_s, 0.0)
+
+
+@dataclass(frozen=True)
+class DenseShape:
+    """pdllm_dense_shape: attention over contiguous K/V (compact static cache, chunk prefill)."""
+    B: int
+    H: int
+    H_kv: int
+    d: int
+    S_pre: int
+    L: int
+    L_s: int
+    scale: float = 0.0
+
+    def c(self) -> PdllmDenseShape:
+        return PdllmDenseShape(self.B, self.H, self.H_kv, self.d, self.S_pre, self.L, self.L_s, self.scale)
+
+    @staticmethod
+    def static_of(shape: "Shape") -> "DenseShape":
+        """The compact-cache attention that corresponds to a Shape (S_pre = K * Bk)."""
+        return DenseShape(shape.B, shape.H, shape.H_kv, shape.d, shape.K * shape.Bk, shape.L, shape.L_s, shape.scale)
 
 
 class PdllmError(RuntimeError):
@@ -98,6 +126,18 @@ def lib() -> ctypes.CDLL:
     L.pdllm_step_profiled.argtypes = [shp, vp, vp, vp, vp, vp, vp, i32, vp, vp, vp, vp, vp, vp, sz,
                                       ctypes.POINTER(PdllmStageEvents), vp]
     L.pdllm_step_host.argtypes = [shp, vp, vp, vp, vp, vp, vp, i32, vp, vp, vp, vp, sz, ctypes.POINTER(PdllmSideStream), vp]
+    dshp = ctypes.POINTER(PdllmDenseShape)
+    L.pdllm_compact_kv.argtypes = [shp, vp, vp, vp, vp, vp, vp, vp]
+    L.pdllm_dense_auto_splits.restype = i32
+    L.pdllm_dense_auto_splits.argtypes = [dshp, i32]
+    L.pdllm_dense_workspace_bytes.restype = sz
+    L.pdllm_dense_workspace_bytes.argtypes = [dshp, i32, i32]
+    L.pdllm_static_attn.argtypes = [dshp, vp, vp, vp, vp, vp, i32, vp, vp, vp, sz, vp]
+    L.pdllm_prefill_attn.argtypes = [dshp, vp, vp, vp, i32, vp, vp, vp, sz, vp]
+    L.pdllm_pool_keys.argtypes = [shp, vp, vp, vp]
+    L.pdllm_score_chunks_pooled.argtypes = [shp, vp, i64, i64, vp, vp, vp]
+    for n in ("pdllm_compact_kv", "pdllm_static_attn", "pdllm_prefill_attn", "pdllm_pool_keys", "pdllm_score_chunks_pooled"):
+        getattr(L, n).restype = ctypes.c_int
     for n in ("pdllm_score_chunks", "pdllm_select_topk", "pdllm_gather_idx", "pdllm_sparse_attn", "pdllm_lse_combine",
               "pdllm_step", "pdllm_step_profiled", "pdllm_step_host"):
         getattr(L, n).restype = ctypes.c_int
@@ -261,3 +301,79 @@ def step_host(shape: Shape, h_Q_dec, h_K_dec, h_V_dec, d_Kcache, d_Vcache, d_tok
     _check(lib().pdllm_step_host(ctypes.byref(shape.c()), _ptr(h_Q_dec), _ptr(h_K_dec), _ptr(h_V_dec), _ptr(d_Kcache),
                                  _ptr(d_Vcache), _ptr(d_token_keep_idx), n_splits, _ptr(h_O), _ptr(h_LSE),
                                  _ptr(h_chunk_ids), _ptr(d_scratch), d_scratch.numel(), sd, _stream(stream)))
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# rows after the hot path
+def compact_kv(shape: Shape, Kcache, Vcache, chunk_ids, token_keep_idx=None, Kcompact=None, Vcompact=None, stream=None):
+    """NEXT-3: the selected, token-thinned rows copied once -> (Kcompact, Vcompact) bf16 [B,H_kv,K*Bk,d]."""
+    torch = _torch()
+    shp = (shape.B, shape.H_kv, shape.K * shape.Bk, shape.d)
+    if Kcompact is None:
+        Kcompact = torch.empty(shp, dtype=torch.bfloat16, device=Kcache.device)
+    if Vcompact is None:
+        Vcompact = torch.empty(shp, dtype=torch.bfloat16, device=Kcache.device)
+    _check(lib().pdllm_compact_kv(ctypes.byref(shape.c()), _ptr(Kcache), _ptr(Vcache), _ptr(chunk_ids), _ptr(token_keep_idx),
+                                  _ptr(Kcompact), _ptr(Vcompact), _stream(stream)))
+    return Kcompact, Vcompact
+
+
+def dense_auto_splits(ds: DenseShape, sms: int = 148) -> int:
+    return lib().pdllm_dense_auto_splits(ctypes.byref(ds.c()), sms)
+
+
+def dense_workspace_bytes(ds: DenseShape, n_splits: int = 0, sms: int = 148) -> int:
+    return lib().pdllm_dense_workspace_bytes(ctypes.byref(ds.c()), n_splits, sms)
+
+
+def alloc_dense_workspace(ds: DenseShape, n_splits: int = 0, device=None):
+    torch = _torch()
+    return torch.empty((max(dense_workspace_bytes(ds, n_splits, num_sms()), 16),), dtype=torch.uint8, device=device or "cuda")
+
+
+def static_attn(ds: DenseShape, Q_dec, Kcompact, Vcompact, K_dec, V_dec, n_splits=0, O=None, LSE=None, workspace=None,
+                stream=None):
+    """NEXT-3: attention over [compact static cache || decode rows], K/V fetched as TMA tiles."""
+    torch = _torch()
+    if O is None:
+        O = torch.empty((ds.B, ds.H, ds.L, ds.d), dtype=torch.bfloat16, device=Q_dec.device)
+    if LSE is None:
+        LSE = torch.empty((ds.B, ds.H, ds.L), dtype=torch.float32, device=Q_dec.device)
+    if workspace is None:
+        workspace = alloc_dense_workspace(ds, n_splits, Q_dec.device)
+    _check(lib().pdllm_static_attn(ctypes.byref(ds.c()), _ptr(Q_dec), _ptr(Kcompact), _ptr(Vcompact), _ptr(K_dec), _ptr(V_dec),
+                                   n_splits, _ptr(O), _ptr(LSE), _ptr(workspace), workspace.numel(), _stream(stream)))
+    return O, LSE
+
+
+def prefill_attn(ds: DenseShape, Q, K, V, n_splits=0, O=None, LSE=None, workspace=None, stream=None):
+    """NEXT-2: bidirectional attention of ds.B independent sequences of T = ds.S_pre = ds.L rows (ds.L_s == 0)."""
+    torch = _torch()
+    if O is None:
+        O = torch.empty((ds.B, ds.H, ds.L, ds.d), dtype=torch.bfloat16, device=Q.device)
+    if LSE is None:
+        LSE = torch.empty((ds.B, ds.H, ds.L), dtype=torch.float32, device=Q.device)
+    if workspace is None:
+        workspace = alloc_dense_workspace(ds, n_splits, Q.device)
+    _check(lib().pdllm_prefill_attn(ctypes.byref(ds.c()), _ptr(Q), _ptr(K), _ptr(V), n_splits, _ptr(O), _ptr(LSE),
+                                    _ptr(workspace), workspace.numel(), _stream(stream)))
+    return O, LSE
+
+
+def pool_keys(shape: Shape, Kcache, kbar=None, stream=None):
+    """NEXT-3 (R23): mean key of every chunk -> fp32 [B,H_kv,N,d]."""
+    torch = _torch()
+    if kbar is None:
+        kbar = torch.empty((shape.B, shape.H_kv, shape.N, shape.d), dtype=torch.float32, device=Kcache.device)
+    _check(lib().pdllm_pool_keys(ctypes.byref(shape.c()), _ptr(Kcache), _ptr(kbar), _stream(stream)))
+    return kbar
+
+
+def score_chunks_pooled(shape: Shape, Q, kbar, scores=None, stream=None):
+    """NEXT-3 (R23): log(C+1) + scale * <mean scoring row, mean key> -> fp32 [B,H_kv,N]."""
+    torch = _torch()
+    if scores is None:
+        scores = torch.empty((shape.B, shape.H_kv, shape.N), dtype=torch.float32, device=Q.device)
+    _check(lib().pdllm_score_chunks_pooled(ctypes.byref(shape.c()), _ptr(Q), Q.stride(0), Q.stride(1), _ptr(kbar),
+                                           _ptr(scores), _stream(stream)))
+    return scores

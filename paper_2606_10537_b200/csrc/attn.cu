@@ -22,6 +22,8 @@
 // second Q buffer to the ring as a sixth slot (its two streams consume four tiles per step).  Ring state is a cursor
 // plus one phase bit per slot, kept alike by the producers and the MMA warp; a slot is released by a tcgen05.commit
 // after its last user (stream 1 in mode A).
+#include <cuda.h>
+
 #include "pdllm_internal.h"
 #include "ptx.cuh"
 
@@ -46,6 +48,7 @@ struct AttnParams {
     float *LSE, *O_part, *lse_part;
     int N, Cp, K, Bk, L_s, S_pre, S_kv, rows_g;
     int n_splits, n_tiles;                                // KV tiles of the whole sequence
+    int contig, T_pre;                                    // contiguous mode: prefix = [B*H_kv, S_pre, d], T_pre tiles of it
     int n_qt, n_pairs, n_single;                          // query tiles per group: n_qt = 2*n_pairs + n_single
     int n_pair_items, n_items;
     int32_t *work_counter;                                // zeroed before launch: next work item to hand out
@@ -57,6 +60,15 @@ struct Item {
     int bg, q0, t0, nt, split;
     bool modeA;
 };
+
+// Valid virtual rows of KV tile `tile`.  Gather mode: one run of S_kv rows.  Contiguous mode (compact static cache,
+// chunk prefill): the prefix and the decode rows are tiled separately -- T_pre prefix tiles, then the decode tiles,
+// each part with its own ragged last tile (softmax attention does not care about the order of its keys).
+__device__ __forceinline__ int tile_valid(const AttnParams &p, int tile) {
+    if (!p.contig) return min(kTileN, p.S_kv - tile * kTileN);
+    if (tile < p.T_pre) return min(kTileN, p.S_pre - tile * kTileN);
+    return min(kTileN, p.L_s - (tile - p.T_pre) * kTileN);
+}
 
 __device__ __forceinline__ Item decode_item(const AttnParams &p, int i) {
     Item it;
@@ -129,7 +141,9 @@ template <int N>
 __device__ __forceinline__ void setmaxnreg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
 
 template <int D>
-__global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams p) {
+__global__ void __launch_bounds__(kAttnThreads, 1)
+attn_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tm_kp, const __grid_constant__ CUtensorMap tm_vp,
+            const __grid_constant__ CUtensorMap tm_kd, const __grid_constant__ CUtensorMap tm_vd) {
     using Cfg = AttnCfg<D>;
     constexpr int ST = Cfg::kStages;
     constexpr int kChunksPerRow = D / 8;                  // 16-byte chunks per row
@@ -257,8 +271,8 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
             const uint16_t *Kd = p.Kd + bg * p.L_s * D, *Vd = p.Vd + bg * p.L_s * D;
             const int32_t *keep = p.keep ? p.keep + bg * p.N * p.Bk : nullptr;
             // the group's K <= 64 chunk ids live in two registers per lane (lane l: ids[l], ids[l + 32])
-            const int ids_lo = lane < p.K ? __ldg(p.ids + bg * p.K + lane) : 0;
-            const int ids_hi = lane + 32 < p.K ? __ldg(p.ids + bg * p.K + lane + 32) : 0;
+            const int ids_lo = (!p.contig && lane < p.K) ? __ldg(p.ids + bg * p.K + lane) : 0;
+            const int ids_hi = (!p.contig && lane + 32 < p.K) ? __ldg(p.ids + bg * p.K + lane + 32) : 0;
             // a3: virtual row -> cache row (>= 0) / decode row (< 0) / invalid; one row per producer thread.  The index
             // is kept as (base, raw) with raw = the keep-list entry still in flight: the sum is only formed when the
             // row is issued, one load later, so the global load latency hides behind the previous tile's cp.async.
@@ -326,7 +340,40 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
                     if (do_v) issue_rows(dst_v, row_addr(my_idx, true), Vc);
                 }
             };
-            if (it.modeA) {
+            // contiguous mode: one thread fetches a whole 128-row tile with 3-D TMA (box 64 x 128 x 1 per 128-byte panel,
+            // rows beyond the part's end read as zeros); the other producer threads only arrive on the tile's barrier
+            auto tma_tile = [&](int tile, int slot, bool is_v) {
+                const uint32_t b = kv_full(slot);
+                if (pt == 0) {
+                    mbar_arrive_expect_tx(b, Cfg::kTileBytes);
+                    const bool pre = tile < p.T_pre;
+                    const CUtensorMap *tm = pre ? (is_v ? &tm_vp : &tm_kp) : (is_v ? &tm_vd : &tm_kd);
+                    const int row0 = (pre ? tile : tile - p.T_pre) * kTileN;
+#pragma unroll
+                    for (int pn = 0; pn < Cfg::kPanels; ++pn)
+                        tma_load_3d(sKV(slot) + pn * Cfg::kPanelBytes, tm, pn * 64, row0, (int)bg, b);
+                } else {
+                    mbar_arrive(b);
+                }
+            };
+            if (p.contig) {
+                load_q();
+                if (it.modeA) {
+                    for (int jt = 0; jt < it.nt; ++jt) {
+                        const int slot_k = take_slot(), slot_v = take_slot();
+                        tma_tile(it.t0 + jt, slot_k, false);
+                        tma_tile(it.t0 + jt, slot_v, true);
+                    }
+                } else {
+                    // the MMA warp's consumption order: K(t0); { K(t0+i+1), V(t0+i) }; V(t0+nt-1)
+                    tma_tile(it.t0, take_slot(), false);
+                    for (int i = 0; i + 1 < it.nt; ++i) {
+                        tma_tile(it.t0 + i + 1, take_slot(), false);
+                        tma_tile(it.t0 + i, take_slot(), true);
+                    }
+                    tma_tile(it.t0 + it.nt - 1, take_slot(), true);
+                }
+            } else if (it.modeA) {
                 // tile by tile, K and V together (one index computation, one cp.async group): loads 2*jt and 2*jt + 1
                 prefetch_index(it.t0);
                 load_q();                                 // Q first: its rows need no indices, the first tile's are in flight
@@ -397,7 +444,7 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
                 return sl;
             };
             auto tile_of = [&](int s, int j) { return it.modeA ? it.t0 + j : it.t0 + 2 * j + s; };
-            auto n_mma_of = [&](int tile) { return (uint32_t)((min(kTileN, p.S_kv - tile * kTileN) + 15) & ~15); };
+            auto n_mma_of = [&](int tile) { return (uint32_t)((tile_valid(p, tile) + 15) & ~15); };
             // the eight SS MMAs of S_s = Q_s K^T and their commits (call from the elected lane only)
             auto emit_qk = [&](int s, int tile, int slot, bool release) {
                 const uint32_t a_lo = lo_k | ((sQ(it.modeA ? s : 0) & 0x3FFFFu) >> 4);
@@ -526,7 +573,7 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
             };
             for (int j = 0; j < n_mine; ++j) {
                 const int tile = it.modeA ? it.t0 + j : it.t0 + 2 * j + s;
-                const int n_valid = min(kTileN, p.S_kv - tile * kTileN);
+                const int n_valid = tile_valid(p, tile);
                 mbar_wait(bar(BAR_SREADY0 + s), n_sready++ & 1u);
                 tc_fence_after();
                 if (__any_sync(0xffffffffu, pend > 0.f)) {
@@ -742,7 +789,7 @@ __global__ void __launch_bounds__(kAttnThreads, 1) attn_kernel(const AttnParams 
 }
 
 template <int D>
-cudaError_t launch_attn_d(const AttnParams &p, cudaStream_t st) {
+cudaError_t launch_attn_d(const AttnParams &p, const CUtensorMap (&tm)[4], cudaStream_t st) {
     using Cfg = AttnCfg<D>;
     cudaError_t e = cudaFuncSetAttribute(attn_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::kSmem);
     if (e != cudaSuccess) return e;
@@ -750,11 +797,33 @@ cudaError_t launch_attn_d(const AttnParams &p, cudaStream_t st) {
     // (Launching this kernel as a programmatic dependent of the top-K kernel was measured -- 2.6 us per step -- and
     // withdrawn: with the combine kernel behind it, long unsynchronised step loops ended in an invalid-address-space
     // fault that a plain launch never shows.)
-    attn_kernel<D><<<grid, kAttnThreads, Cfg::kSmem, st>>>(p);
+    attn_kernel<D><<<grid, kAttnThreads, Cfg::kSmem, st>>>(p, tm[0], tm[1], tm[2], tm[3]);
     return cudaGetLastError();
 }
 
+void fill_common(AttnParams &p, const Dims &s, int n_splits) {
+    p.N = s.N; p.Cp = s.Cp; p.K = s.K; p.Bk = s.Bk; p.L_s = s.L_s;
+    p.S_pre = s.S_pre; p.S_kv = s.S_kv; p.rows_g = s.rows_g;
+    p.contig = s.contig;
+    p.T_pre = (s.S_pre + kTileN - 1) / kTileN;
+    p.n_tiles = kv_tiles(s);
+    p.n_splits = n_splits;
+    p.n_qt = (s.rows_g + kTileM - 1) / kTileM;
+    p.n_pairs = p.n_qt / 2;
+    p.n_single = p.n_qt & 1;
+    const int BG = s.B * s.H_kv;
+    p.n_pair_items = BG * p.n_pairs * n_splits;
+    p.n_items = p.n_pair_items + BG * p.n_single * n_splits;
+    p.total_rows = (int64_t)s.B * s.H * s.L;
+    p.c2 = s.scale * 1.4426950408889634f;
+}
+
 }  // namespace
+
+int kv_tiles(const Dims &d) {
+    if (!d.contig) return (d.S_kv + kTileN - 1) / kTileN;
+    return (d.S_pre + kTileN - 1) / kTileN + (d.L_s + kTileN - 1) / kTileN;
+}
 
 cudaError_t launch_attn(const Dims &s, const void *Q_dec, const void *Kcache, const void *Vcache, const int32_t *chunk_ids,
                         const int32_t *keep, const void *K_dec, const void *V_dec, int n_splits, void *O, float *LSE,
@@ -772,19 +841,22 @@ cudaError_t launch_attn(const Dims &s, const void *Q_dec, const void *Kcache, co
     p.O_part = O_part;
     p.lse_part = lse_part;
     p.work_counter = work_counter;
-    p.N = s.N; p.Cp = s.Cp; p.K = s.K; p.Bk = s.Bk; p.L_s = s.L_s;
-    p.S_pre = s.S_pre; p.S_kv = s.S_kv; p.rows_g = s.rows_g;
-    p.n_tiles = (s.S_kv + kTileN - 1) / kTileN;
-    p.n_splits = n_splits;
-    p.n_qt = (s.rows_g + kTileM - 1) / kTileM;
-    p.n_pairs = p.n_qt / 2;
-    p.n_single = p.n_qt & 1;
-    const int BG = s.B * s.H_kv;
-    p.n_pair_items = BG * p.n_pairs * n_splits;
-    p.n_items = p.n_pair_items + BG * p.n_single * n_splits;
-    p.total_rows = (int64_t)s.B * s.H * s.L;
-    p.c2 = s.scale * 1.4426950408889634f;
-    return s.d == 128 ? launch_attn_d<128>(p, st) : launch_attn_d<64>(p, st);
+    fill_common(p, s, n_splits);
+    CUtensorMap tm[4];
+    if (s.contig) {
+        // contiguous mode: Kcache / Vcache are [B*H_kv, S_pre, d] (compact static cache, or a prefill sequence's K / V);
+        // K_dec / V_dec [B*H_kv, L_s, d] may be absent (L_s == 0)
+        const uint64_t BG = (uint64_t)s.B * s.H_kv;
+        const bool dec = s.L_s > 0;
+        if (!make_rows_tmap3d(&tm[0], Kcache, BG, (uint64_t)s.S_pre, s.d, kTileN) ||
+            !make_rows_tmap3d(&tm[1], Vcache, BG, (uint64_t)s.S_pre, s.d, kTileN) ||
+            !make_rows_tmap3d(&tm[2], dec ? K_dec : Kcache, BG, (uint64_t)(dec ? s.L_s : s.S_pre), s.d, kTileN) ||
+            !make_rows_tmap3d(&tm[3], dec ? V_dec : Vcache, BG, (uint64_t)(dec ? s.L_s : s.S_pre), s.d, kTileN))
+            return cudaErrorInvalidValue;
+    } else {
+        memset(tm, 0, sizeof(tm));
+    }
+    return s.d == 128 ? launch_attn_d<128>(p, tm, st) : launch_attn_d<64>(p, tm, st);
 }
 
 }  // namespace pdllm

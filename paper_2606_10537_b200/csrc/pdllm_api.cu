@@ -50,11 +50,10 @@ int resolve(const pdllm_shape *sh, bool has_keep, Dims *out) {
     d.S_pre = sh->K * sh->Bk; d.S_kv = d.S_pre + sh->L_s;
     d.rows_g = d.G * sh->L;
     d.scale = sh->scale > 0.f ? sh->scale : 1.0f / std::sqrt((float)sh->d);
+    d.contig = 0;
     *out = d;
     return PDLLM_OK;
 }
-
-int kv_tiles(const Dims &d) { return (d.S_kv + kTileN - 1) / kTileN; }
 
 // a6: the attention kernel runs one persistent CTA per SM over work items (attn.cu): per KV group and split,
 // floor(n_qt/2) pair items (both streams walk the split's tiles: ceil(T/S) steps) and n_qt%2 single items (the two
@@ -296,6 +295,106 @@ int pdllm_sparse_attn(const pdllm_shape *shape, const void *Q_dec, const void *K
     if (int rc = debug_validate(d, chunk_ids, token_keep_idx, static_cast<cudaStream_t>(stream))) return rc;
     return attn_impl(d, Q_dec, Kcache, Vcache, chunk_ids, token_keep_idx, K_dec, V_dec, S, O, LSE, gather_idx_out,
                      workspace, false, nullptr, nullptr, static_cast<cudaStream_t>(stream));
+}
+
+// ---- the static-selection fast path and the chunk prefill: attention over contiguous K/V (TMA tiles)
+namespace {
+
+int resolve_dense(const pdllm_dense_shape *sh, Dims *out) {
+    if (!sh) return PDLLM_ERR_NULL;
+    if (sh->B < 1 || sh->H < 1 || sh->H_kv < 1 || sh->H % sh->H_kv != 0) return PDLLM_ERR_SHAPE;
+    if (sh->d != 64 && sh->d != 128) return PDLLM_ERR_SHAPE;
+    if (sh->S_pre < 1 || sh->L < 1 || sh->L_s < 0) return PDLLM_ERR_SHAPE;
+    if ((int64_t)sh->S_pre + sh->L_s >= (1ll << 30) || (int64_t)sh->B * sh->H_kv > 65535) return PDLLM_ERR_SHAPE;
+    Dims d;
+    memset(&d, 0, sizeof d);
+    d.B = sh->B; d.H = sh->H; d.H_kv = sh->H_kv; d.G = sh->H / sh->H_kv; d.d = sh->d;
+    d.N = 1; d.C = sh->S_pre - 1; d.Cp = sh->S_pre; d.K = 1; d.Bk = sh->S_pre;
+    d.L_q = 1; d.L = sh->L; d.L_s = sh->L_s;
+    d.S_pre = sh->S_pre; d.S_kv = sh->S_pre + sh->L_s;
+    d.rows_g = d.G * sh->L;
+    d.scale = sh->scale > 0.f ? sh->scale : 1.0f / std::sqrt((float)sh->d);
+    d.contig = 1;
+    *out = d;
+    return PDLLM_OK;
+}
+
+int dense_attn(const pdllm_dense_shape *shape, const void *Q, const void *Kpre, const void *Vpre, const void *K_dec,
+               const void *V_dec, int32_t n_splits, void *O, float *LSE, void *workspace, size_t workspace_bytes,
+               pdllm_stream_t stream) {
+    if (!shape || !Q || !Kpre || !Vpre || !O || !LSE) return PDLLM_ERR_NULL;
+    if (n_splits < 0) return PDLLM_ERR_SHAPE;
+    Dims d;
+    if (int rc = resolve_dense(shape, &d)) return rc;
+    if (d.L_s > 0 && (!K_dec || !V_dec)) return PDLLM_ERR_NULL;
+    if (!aligned16(Q) || !aligned16(Kpre) || !aligned16(Vpre) || !aligned16(O) || !aligned16(workspace) ||
+        (d.L_s > 0 && (!aligned16(K_dec) || !aligned16(V_dec))))
+        return PDLLM_ERR_ALIGN;
+    int S = effective_splits(d, n_splits, device_num_sms());
+    if (!workspace) return PDLLM_ERR_WORKSPACE;
+    if (n_splits == 0)
+        while (S > 1 && workspace_bytes < workspace_for(d, S)) --S;
+    if (workspace_bytes < workspace_for(d, S)) return PDLLM_ERR_WORKSPACE;
+    return attn_impl(d, Q, Kpre, Vpre, nullptr, nullptr, K_dec, V_dec, S, O, LSE, nullptr, workspace, false, nullptr,
+                     nullptr, static_cast<cudaStream_t>(stream));
+}
+
+}  // namespace
+
+size_t pdllm_dense_workspace_bytes(const pdllm_dense_shape *shape, int32_t n_splits, int32_t num_sms) {
+    Dims d;
+    if (n_splits < 0 || resolve_dense(shape, &d) != PDLLM_OK) return 0;
+    return workspace_for(d, effective_splits(d, n_splits, num_sms));
+}
+
+int32_t pdllm_dense_auto_splits(const pdllm_dense_shape *shape, int32_t num_sms) {
+    Dims d;
+    if (resolve_dense(shape, &d) != PDLLM_OK) return 1;
+    return effective_splits(d, 0, num_sms);
+}
+
+int pdllm_compact_kv(const pdllm_shape *shape, const void *Kcache, const void *Vcache, const int32_t *chunk_ids,
+                     const int32_t *token_keep_idx, void *Kcompact, void *Vcompact, pdllm_stream_t stream) {
+    if (!shape || !Kcache || !Vcache || !chunk_ids || !Kcompact || !Vcompact) return PDLLM_ERR_NULL;
+    Dims d;
+    if (int rc = resolve(shape, token_keep_idx != nullptr, &d)) return rc;
+    if (!aligned16(Kcache) || !aligned16(Vcache) || !aligned16(Kcompact) || !aligned16(Vcompact)) return PDLLM_ERR_ALIGN;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (int rc = debug_validate(d, chunk_ids, token_keep_idx, st)) return rc;
+    return cuda_rc(launch_compact_kv(d, Kcache, Vcache, chunk_ids, token_keep_idx, Kcompact, Vcompact, st));
+}
+
+int pdllm_static_attn(const pdllm_dense_shape *shape, const void *Q_dec, const void *Kcompact, const void *Vcompact,
+                      const void *K_dec, const void *V_dec, int32_t n_splits, void *O, float *LSE, void *workspace,
+                      size_t workspace_bytes, pdllm_stream_t stream) {
+    return dense_attn(shape, Q_dec, Kcompact, Vcompact, K_dec, V_dec, n_splits, O, LSE, workspace, workspace_bytes, stream);
+}
+
+int pdllm_prefill_attn(const pdllm_dense_shape *shape, const void *Q, const void *K, const void *V, int32_t n_splits,
+                       void *O, float *LSE, void *workspace, size_t workspace_bytes, pdllm_stream_t stream) {
+    if (shape && (shape->L_s != 0 || shape->L != shape->S_pre)) return PDLLM_ERR_SHAPE;
+    return dense_attn(shape, Q, K, V, nullptr, nullptr, n_splits, O, LSE, workspace, workspace_bytes, stream);
+}
+
+int pdllm_pool_keys(const pdllm_shape *shape, const void *Kcache, float *kbar, pdllm_stream_t stream) {
+    if (!shape || !Kcache || !kbar) return PDLLM_ERR_NULL;
+    Dims d;
+    pdllm_shape sh = *shape;
+    sh.Bk = sh.C + 1;
+    if (int rc = resolve(&sh, false, &d)) return rc;
+    if (!aligned16(Kcache) || !aligned16(kbar)) return PDLLM_ERR_ALIGN;
+    return cuda_rc(launch_pool_keys(d, Kcache, kbar, static_cast<cudaStream_t>(stream)));
+}
+
+int pdllm_score_chunks_pooled(const pdllm_shape *shape, const void *Q, int64_t q_batch_stride, int64_t q_head_stride,
+                              const float *kbar, float *scores, pdllm_stream_t stream) {
+    if (!shape || !Q || !kbar || !scores) return PDLLM_ERR_NULL;
+    Dims d;
+    pdllm_shape sh = *shape;
+    sh.Bk = sh.C + 1;
+    if (int rc = resolve(&sh, false, &d)) return rc;
+    if (q_head_stride < (int64_t)d.L_q * d.d) return PDLLM_ERR_ALIGN;
+    return cuda_rc(launch_pooled_scores(d, Q, q_batch_stride, q_head_stride, kbar, scores, static_cast<cudaStream_t>(stream)));
 }
 
 int pdllm_step_profiled(const pdllm_shape *shape, const void *Q_dec, const void *Kcache, const void *Vcache,

@@ -1,8 +1,10 @@
 // pdllm_internal.h -- declarations shared by the translation units of libpdllm.so (not installed).
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <cstddef>
 #include <cstdint>
+#include <cstring>
 
 #include "../../include/pdllm.h"
 
@@ -16,6 +18,7 @@ struct Dims {
     int S_pre, S_kv;      // K*Bk, K*Bk + L_s
     int rows_g;           // G*L: rows of Q_dec that share one KV head (contiguous in [B,H,L,d])
     float scale;
+    int contig;           // 1: the prefix is a contiguous [B*H_kv, S_pre, d] cache (compact static cache / chunk prefill)
 };
 
 constexpr int kTileM = 128;   // query rows per CTA tile (UMMA M)
@@ -41,5 +44,20 @@ cudaError_t launch_attn(const Dims &s, const void *Q_dec, const void *Kcache, co
                         float *O_part, float *lse_part, int32_t *work_counter, cudaStream_t st);
 
 int device_num_sms();
+// KV tiles of 128 rows one query tile walks (gather mode: ceil(S_kv / 128); contiguous mode: prefix and decode rows
+// are tiled separately)
+int kv_tiles(const Dims &d);
+
+// TMA descriptors (score.cu): bf16 [rows, d] row-major, box = [box_rows, 64 columns], 128-byte swizzle, OOB rows read as
+// zero; the 3-D form adds an outermost index over `groups` matrices of `rows` rows each.
+bool make_rows_tmap(CUtensorMap *tm, const void *base, uint64_t rows, int d, int box_rows);
+bool make_rows_tmap3d(CUtensorMap *tm, const void *base, uint64_t groups, uint64_t rows, int d, int box_rows);
+
+// ---- NEXT-3 (static_cache.cu)
+cudaError_t launch_compact_kv(const Dims &s, const void *Kcache, const void *Vcache, const int32_t *chunk_ids,
+                              const int32_t *keep, void *Kcompact, void *Vcompact, cudaStream_t st);
+cudaError_t launch_pool_keys(const Dims &s, const void *Kcache, float *kbar, cudaStream_t st);
+cudaError_t launch_pooled_scores(const Dims &s, const void *Q, int64_t q_batch_stride, int64_t q_head_stride,
+                                 const float *kbar, float *scores, cudaStream_t st);
 
 }  // namespace pdllm

@@ -109,6 +109,13 @@ __device__ __forceinline__ void tma_load_2d(uint32_t dst, const void *tmap, int3
         ::"r"(dst), "l"(tmap), "r"(c0), "r"(c1), "r"(bar)
         : "memory");
 }
+// 3-D tiled load: box at (c0 = innermost column, c1 = row, c2 = outermost index)
+__device__ __forceinline__ void tma_load_3d(uint32_t dst, const void *tmap, int32_t c0, int32_t c1, int32_t c2, uint32_t bar) {
+    asm volatile(
+        "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
+        ::"r"(dst), "l"(tmap), "r"(c0), "r"(c1), "r"(c2), "r"(bar)
+        : "memory");
+}
 __device__ __forceinline__ void tma_load_2d_hint(uint32_t dst, const void *tmap, int32_t c0, int32_t c1, uint32_t bar,
                                                  uint64_t policy) {
     asm volatile(

@@ -341,6 +341,8 @@ EncodeTiledFn encode_tiled_fn() {
     return fn;
 }
 
+}  // namespace
+
 // bf16 [rows, d] row-major, box = [box_rows, 64 columns], 128-byte swizzle, OOB rows read as zero.
 bool make_rows_tmap(CUtensorMap *tm, const void *base, uint64_t rows, int d, int box_rows) {
     EncodeTiledFn fn = encode_tiled_fn();
@@ -353,6 +355,20 @@ bool make_rows_tmap(CUtensorMap *tm, const void *base, uint64_t rows, int d, int
               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
+
+bool make_rows_tmap3d(CUtensorMap *tm, const void *base, uint64_t groups, uint64_t rows, int d, int box_rows) {
+    EncodeTiledFn fn = encode_tiled_fn();
+    if (!fn) return false;
+    cuuint64_t dims[3] = {(cuuint64_t)d, rows, groups};
+    cuuint64_t strides[2] = {(cuuint64_t)d * 2, (cuuint64_t)d * 2 * rows};
+    cuuint32_t box[3] = {64, (cuuint32_t)box_rows, 1};
+    cuuint32_t es[3] = {1, 1, 1};
+    return fn(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void *>(base), dims, strides, box, es,
+              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+namespace {
 
 template <int D>
 cudaError_t launch_score_d(const ScoreParams &p, const CUtensorMap &t128, const CUtensorMap &t16, int BG, cudaStream_t st) {
