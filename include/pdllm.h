@@ -291,6 +291,32 @@ int pdllm_score_chunks_pooled(const pdllm_shape *shape, const void *Q, int64_t q
                               int64_t q_head_stride, const float *kbar, float *scores,
                               pdllm_stream_t stream);
 
+/* ---- NEXT-1: intra-chunk token eviction scores and top-B retention ---------------
+ * (Eq. 5, the query->chunk term -- Table 7's "query-to-chunk" variant,
+ * P:457-465; "only the top-B KV entries per chunk are retained"; R7, R22.)
+ * The step just before the hot path: it produces token_keep_idx on the device.
+ *
+ * pdllm_score_tokens:
+ *   e[b,g,n,j] = sum over the G*L_q scoring rows (h in group g, i < L_q) of
+ *                softmax_j( scale * <Q[b,h,i,:], Kcache[b,g,n,j,:]> ),
+ * the softmax running over the chunk's own C+1 slots (the cache holds no query or
+ * pseudo-label keys: R22; parity unpinned by the paper).  Every chunk's slots sum
+ * to G*L_q.  Two streaming passes over the K cache (row log-masses, then scores).
+ *   Q, strides, Kcache as in pdllm_score_chunks;
+ *   token_scores device fp32 [B,H_kv,N,C+1] (out);
+ *   workspace   device scratch >= pdllm_score_tokens_workspace_bytes(shape)
+ * pdllm_select_topb: per chunk slot 0 (BOS, always) and the Bk-1 slots of 1..C with
+ * the highest score, ties to the lower slot, NaN as -inf, emitted ascending --
+ * exactly the list pdllm_sparse_attn / pdllm_step / pdllm_compact_kv take.
+ *   token_scores device fp32 [B,H_kv,N,C+1]; token_keep_idx device int32 [B,H_kv,N,Bk] (out);
+ *   C + 1 <= 8192, else PDLLM_ERR_UNSUPPORTED                                       */
+size_t pdllm_score_tokens_workspace_bytes(const pdllm_shape *shape);
+int pdllm_score_tokens(const pdllm_shape *shape, const void *Q, int64_t q_batch_stride,
+                       int64_t q_head_stride, const void *Kcache, float *token_scores,
+                       void *workspace, size_t workspace_bytes, pdllm_stream_t stream);
+int pdllm_select_topb(const pdllm_shape *shape, const float *token_scores, int32_t *token_keep_idx,
+                      pdllm_stream_t stream);
+
 /* ---- NEXT-2: attention of the chunk prefill (Eq. 2; Fig. 5(a)) --
  * Each of the shape->B = B*N sequences [BOS; c_i; q; m] (T = S_pre = L rows, L_s = 0)
  * attends to itself, bidirectionally and unmasked, independently of all

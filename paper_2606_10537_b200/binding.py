@@ -24,6 +24,7 @@ EXPORTS = [
     # rows after the hot path
     "pdllm_compact_kv", "pdllm_dense_auto_splits", "pdllm_dense_workspace_bytes", "pdllm_static_attn",
     "pdllm_pool_keys", "pdllm_score_chunks_pooled", "pdllm_prefill_attn",
+    "pdllm_score_tokens_workspace_bytes", "pdllm_score_tokens", "pdllm_select_topb",
 ]
 
 
@@ -136,6 +137,12 @@ def lib() -> ctypes.CDLL:
     L.pdllm_prefill_attn.argtypes = [dshp, vp, vp, vp, i32, vp, vp, vp, sz, vp]
     L.pdllm_pool_keys.argtypes = [shp, vp, vp, vp]
     L.pdllm_score_chunks_pooled.argtypes = [shp, vp, i64, i64, vp, vp, vp]
+    L.pdllm_score_tokens_workspace_bytes.restype = sz
+    L.pdllm_score_tokens_workspace_bytes.argtypes = [shp]
+    L.pdllm_score_tokens.argtypes = [shp, vp, i64, i64, vp, vp, vp, sz, vp]
+    L.pdllm_select_topb.argtypes = [shp, vp, vp, vp]
+    L.pdllm_score_tokens.restype = ctypes.c_int
+    L.pdllm_select_topb.restype = ctypes.c_int
     for n in ("pdllm_compact_kv", "pdllm_static_attn", "pdllm_prefill_attn", "pdllm_pool_keys", "pdllm_score_chunks_pooled"):
         getattr(L, n).restype = ctypes.c_int
     for n in ("pdllm_score_chunks", "pdllm_select_topk", "pdllm_gather_idx", "pdllm_sparse_attn", "pdllm_lse_combine",
@@ -377,3 +384,26 @@ def score_chunks_pooled(shape: Shape, Q, kbar, scores=None, stream=None):
     _check(lib().pdllm_score_chunks_pooled(ctypes.byref(shape.c()), _ptr(Q), Q.stride(0), Q.stride(1), _ptr(kbar),
                                            _ptr(scores), _stream(stream)))
     return scores
+
+
+def score_tokens(shape: Shape, Q, Kcache, token_scores=None, workspace=None, stream=None):
+    """NEXT-1: token eviction scores (Eq. 5, query->chunk) -> fp32 [B,H_kv,N,C+1]."""
+    torch = _torch()
+    if token_scores is None:
+        token_scores = torch.empty((shape.B, shape.H_kv, shape.N, shape.C + 1), dtype=torch.float32, device=Q.device)
+    if workspace is None:
+        nbytes = lib().pdllm_score_tokens_workspace_bytes(ctypes.byref(shape.c()))
+        workspace = torch.empty((max(nbytes, 16),), dtype=torch.uint8, device=Q.device)
+    assert Q.is_contiguous() and Kcache.is_contiguous()
+    _check(lib().pdllm_score_tokens(ctypes.byref(shape.c()), _ptr(Q), Q.stride(0), Q.stride(1), _ptr(Kcache),
+                                    _ptr(token_scores), _ptr(workspace), workspace.numel(), _stream(stream)))
+    return token_scores
+
+
+def select_topb(shape: Shape, token_scores, token_keep_idx=None, stream=None):
+    """NEXT-1: per chunk BOS + the Bk-1 best slots, ascending -> int32 [B,H_kv,N,Bk]."""
+    torch = _torch()
+    if token_keep_idx is None:
+        token_keep_idx = torch.empty((shape.B, shape.H_kv, shape.N, shape.Bk), dtype=torch.int32, device=token_scores.device)
+    _check(lib().pdllm_select_topb(ctypes.byref(shape.c()), _ptr(token_scores), _ptr(token_keep_idx), _stream(stream)))
+    return token_keep_idx

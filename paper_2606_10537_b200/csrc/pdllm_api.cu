@@ -201,7 +201,7 @@ int pdllm_score_chunks(const pdllm_shape *shape, const void *Q, int64_t q_batch_
     if (int rc = resolve(&sh, false, &d)) return rc;
     if (!aligned16(Q) || !aligned16(Kcache) || !aligned16(scores)) return PDLLM_ERR_ALIGN;
     if ((q_batch_stride & 7) || (q_head_stride & 7) || q_head_stride < (int64_t)d.L_q * d.d) return PDLLM_ERR_ALIGN;
-    return cuda_rc(launch_score(d, Q, q_batch_stride, q_head_stride, Kcache, scores, static_cast<cudaStream_t>(stream)));
+    return cuda_rc(launch_score(d, Q, q_batch_stride, q_head_stride, Kcache, scores, nullptr, static_cast<cudaStream_t>(stream)));
 }
 
 int pdllm_select_topk(const pdllm_shape *shape, const float *scores, int32_t *chunk_ids, pdllm_stream_t stream) {
@@ -376,6 +376,63 @@ int pdllm_prefill_attn(const pdllm_dense_shape *shape, const void *Q, const void
     return dense_attn(shape, Q, K, V, nullptr, nullptr, n_splits, O, LSE, workspace, workspace_bytes, stream);
 }
 
+// ---- NEXT-1: token eviction scores and top-B retention
+namespace {
+struct TokScratch { size_t scores, row_lse, part, total; };
+TokScratch tok_scratch(const Dims &d) {
+    TokScratch t;
+    size_t off = 0;
+    auto take = [&](size_t bytes) { size_t o = off; off += align_up(bytes, 256); return o; };
+    const size_t BG = (size_t)d.B * d.H_kv, rows = (size_t)d.G * d.L_q, m_tiles = (rows + kTileM - 1) / kTileM;
+    t.scores = take(BG * d.N * sizeof(float));
+    t.row_lse = take(BG * d.N * rows * sizeof(float));
+    t.part = off;
+    if (m_tiles > 1) take(m_tiles * BG * d.N * d.Cp * sizeof(float));
+    t.total = off;
+    return t;
+}
+}  // namespace
+
+size_t pdllm_score_tokens_workspace_bytes(const pdllm_shape *shape) {
+    if (!shape) return 0;
+    Dims d;
+    pdllm_shape sh = *shape;
+    sh.Bk = sh.C + 1;
+    if (resolve(&sh, false, &d) != PDLLM_OK) return 0;
+    return tok_scratch(d).total;
+}
+
+int pdllm_score_tokens(const pdllm_shape *shape, const void *Q, int64_t q_batch_stride, int64_t q_head_stride,
+                       const void *Kcache, float *token_scores, void *workspace, size_t workspace_bytes,
+                       pdllm_stream_t stream) {
+    if (!shape || !Q || !Kcache || !token_scores || !workspace) return PDLLM_ERR_NULL;
+    Dims d;
+    pdllm_shape sh = *shape;
+    sh.Bk = sh.C + 1;
+    if (int rc = resolve(&sh, false, &d)) return rc;
+    if (!aligned16(Q) || !aligned16(Kcache) || !aligned16(token_scores) || !aligned16(workspace)) return PDLLM_ERR_ALIGN;
+    if ((q_batch_stride & 7) || (q_head_stride & 7) || q_head_stride < (int64_t)d.L_q * d.d) return PDLLM_ERR_ALIGN;
+    const TokScratch t = tok_scratch(d);
+    if (workspace_bytes < t.total) return PDLLM_ERR_WORKSPACE;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    char *base = static_cast<char *>(workspace);
+    float *row_lse = reinterpret_cast<float *>(base + t.row_lse);
+    // pass 1: the chunk-score kernel exports every scoring row's log-mass per chunk; pass 2: the token kernel
+    if (int rc = cuda_rc(launch_score(d, Q, q_batch_stride, q_head_stride, Kcache, reinterpret_cast<float *>(base + t.scores),
+                                      row_lse, st)))
+        return rc;
+    return cuda_rc(launch_token_scores(d, Q, q_batch_stride, q_head_stride, Kcache, row_lse, token_scores,
+                                       reinterpret_cast<float *>(base + t.part), st));
+}
+
+int pdllm_select_topb(const pdllm_shape *shape, const float *token_scores, int32_t *token_keep_idx, pdllm_stream_t stream) {
+    if (!shape || !token_scores || !token_keep_idx) return PDLLM_ERR_NULL;
+    Dims d;
+    if (int rc = resolve(shape, true, &d)) return rc;
+    if (d.Cp > topb_max_cp()) return PDLLM_ERR_UNSUPPORTED;
+    return cuda_rc(launch_topb(d, token_scores, token_keep_idx, static_cast<cudaStream_t>(stream)));
+}
+
 int pdllm_pool_keys(const pdllm_shape *shape, const void *Kcache, float *kbar, pdllm_stream_t stream) {
     if (!shape || !Kcache || !kbar) return PDLLM_ERR_NULL;
     Dims d;
@@ -415,7 +472,7 @@ int pdllm_step_profiled(const pdllm_shape *shape, const void *Q_dec, const void 
     // the attention's work-item counter is cleared here, far ahead of its kernel (off the step's critical path)
     if (int rc = cuda_rc(cudaMemsetAsync(workspace, 0, sizeof(int32_t), st))) return rc;
     if (int rc = record(ev ? ev->begin : nullptr, st)) return rc;
-    if (int rc = cuda_rc(launch_score(d, Q_dec, (int64_t)d.H * d.L * d.d, (int64_t)d.L * d.d, Kcache, scores_out, st)))
+    if (int rc = cuda_rc(launch_score(d, Q_dec, (int64_t)d.H * d.L * d.d, (int64_t)d.L * d.d, Kcache, scores_out, nullptr, st)))
         return rc;
     if (int rc = record(ev ? ev->after_score : nullptr, st)) return rc;
     if (int rc = cuda_rc(launch_topk(d, scores_out, chunk_ids_out, st))) return rc;
@@ -474,7 +531,7 @@ int pdllm_step_host(const pdllm_shape *shape, const void *h_Q_dec, const void *h
     if (cudaMemcpyAsync(base + h.vd, h_V_dec, kb, cudaMemcpyHostToDevice, st2) != cudaSuccess) return PDLLM_ERR_CUDA;
     if (side && cudaEventRecord(ev_join, st2) != cudaSuccess) return PDLLM_ERR_CUDA;
     if (int rc = cuda_rc(cudaMemsetAsync(base + h.ws, 0, sizeof(int32_t), st))) return rc;
-    if (int rc = cuda_rc(launch_score(dv, base + h.q, (int64_t)dv.H * dv.L * dv.d, (int64_t)dv.L * dv.d, d_Kcache, scores, st)))
+    if (int rc = cuda_rc(launch_score(dv, base + h.q, (int64_t)dv.H * dv.L * dv.d, (int64_t)dv.L * dv.d, d_Kcache, scores, nullptr, st)))
         return rc;
     if (int rc = cuda_rc(launch_topk(dv, scores, ids, st))) return rc;
     if (side && cudaStreamWaitEvent(st, ev_join, 0) != cudaSuccess) return PDLLM_ERR_CUDA;

@@ -35,8 +35,14 @@ cudaError_t launch_validate(const Dims &s, const int32_t *chunk_ids, const int32
 cudaError_t launch_combine(const float *O_part, const float *lse_part, int S, int64_t rows, int d, void *O, float *LSE,
                            cudaStream_t st);
 // ---- a1: scores[b,g,n]
+// row_lse (optional): [B*H_kv, N, G*L_q] fp32, every scoring row's log-mass per chunk
 cudaError_t launch_score(const Dims &s, const void *Q, int64_t q_batch_stride, int64_t q_head_stride, const void *Kcache,
-                         float *scores, cudaStream_t st);
+                         float *scores, float *row_lse, cudaStream_t st);
+// ---- NEXT-1 (token_score.cu): e [B,H_kv,N,Cp] from row_lse; e_part: [m_tiles, B,H_kv,N,Cp] scratch when G*L_q > 128
+cudaError_t launch_token_scores(const Dims &s, const void *Q, int64_t q_batch_stride, int64_t q_head_stride,
+                                const void *Kcache, const float *row_lse, float *e, float *e_part, cudaStream_t st);
+cudaError_t launch_topb(const Dims &s, const float *token_scores, int32_t *keep, cudaStream_t st);
+int topb_max_cp();
 // ---- a3+a4 into O / LSE (n_splits == 1) or into the partials (n_splits > 1: launch_combine follows);
 // work_counter: one zeroed int32 (the persistent kernel's work-item counter)
 cudaError_t launch_attn(const Dims &s, const void *Q_dec, const void *Kcache, const void *Vcache, const int32_t *chunk_ids,

@@ -28,6 +28,7 @@ struct ScoreParams {
     const uint16_t *Q;
     int64_t q_batch_stride, q_head_stride;
     float *scores;
+    float *row_lse;                       // optional export [B*H_kv, N, rows]: every scoring row's log-mass per chunk (NEXT-1)
     int H_kv, G, N, Cp, L_q, rows;        // rows = G * L_q
     int m_tiles;
     int64_t units;                        // (b, g, M tile, chunk) work units, split evenly over the persistent CTAs
@@ -303,6 +304,7 @@ score_kernel(const ScoreParams p, const __grid_constant__ CUtensorMap tmap128, c
                 const float m = fmaxf(m_ref, m1);
                 const float lt = l * ex2_approx(m_ref - m) + (l1 > 0.f ? l1 * ex2_approx(m1 - m) : 0.f);
                 float ell = row_ok ? (m + lg2_approx(lt)) * 0.6931471805599453f : 0.f;
+                if (p.row_lse && row_ok) p.row_lse[((int64_t)bg * p.N + n) * p.rows + mt * kTileM + row] = ell;
 #pragma unroll
                 for (int o = 16; o > 0; o >>= 1) ell += __shfl_xor_sync(0xffffffffu, ell, o);
                 if (lane == 0) s_acc[(n - n0) * 4 + warp] = ell;
@@ -384,12 +386,13 @@ cudaError_t launch_score_d(const ScoreParams &p, const CUtensorMap &t128, const 
 }  // namespace
 
 cudaError_t launch_score(const Dims &s, const void *Q, int64_t q_batch_stride, int64_t q_head_stride, const void *Kcache,
-                         float *scores, cudaStream_t st) {
+                         float *scores, float *row_lse, cudaStream_t st) {
     ScoreParams p;
     p.Q = static_cast<const uint16_t *>(Q);
     p.q_batch_stride = q_batch_stride;
     p.q_head_stride = q_head_stride;
     p.scores = scores;
+    p.row_lse = row_lse;
     p.H_kv = s.H_kv; p.G = s.G; p.N = s.N; p.Cp = s.Cp; p.L_q = s.L_q;
     p.rows = s.G * s.L_q;
     p.m_tiles = (p.rows + kTileM - 1) / kTileM;

@@ -39,8 +39,12 @@ class Workload:
     alpha: float         # planted key shift, in units of mean(q) (R20)
     unit_logits: bool    # True: Q,K,V ~ N(0,1)/sqrt(d) (config "tiny"); False: N(0,1)
     seed: int
-    token_alpha: float = 0.0   # > 0 (NEXT-1 workloads only): the keys of the slots on the keep list are shifted by
-                               # token_alpha * mean(q) in every chunk, so that top-B token retention has a clear gap
+    # NEXT-1 workloads only -- planted tokens, so that top-B token retention has a clear gap: in every chunk the keys of
+    # the slots on the keep list are shifted by token_alpha * mean(q) (works while G*L_q is small enough for the rows to
+    # agree with their mean: config "tiny") and / or multiplied by token_gamma (a longer key draws more softmax mass from
+    # every row whatever its direction: the N(0,1) configs)
+    token_alpha: float = 0.0
+    token_gamma: float = 1.0
 
     @property
     def G(self): return self.H // self.H_kv
@@ -156,8 +160,9 @@ def make_inputs(w: Workload, threads: int = 8) -> dict:
         b, g = divmod(bg, w.H_kv)
         k = _normal(w.seed, T_KC, bg, (w.N, w.Cp, w.d), sigma)
         k[planted[b, g]] += np.float32(w.alpha) * qbar[b, g]        # shift every row of the planted chunks
-        if w.token_alpha > 0.0 and keep is not None:                  # planted tokens: the kept slots of every chunk
-            k[np.arange(w.N)[:, None], keep[b, g, :, 1:]] += np.float32(w.token_alpha) * qbar[b, g]
+        if keep is not None and (w.token_alpha > 0.0 or w.token_gamma != 1.0):      # planted tokens: the kept slots
+            sel = (np.arange(w.N)[:, None], keep[b, g, :, 1:])
+            k[sel] = k[sel] * np.float32(w.token_gamma) + np.float32(w.token_alpha) * qbar[b, g]
         Kc[b, g] = f32_to_bf16_bits(k)
         Vc[b, g] = f32_to_bf16_bits(_normal(w.seed, T_VC, bg, (w.N, w.Cp, w.d), sigma))
 

@@ -130,3 +130,87 @@ def test_prefill_attn(B, S, H, H_kv, T, d, splits):
         e_o, r_o = check_O(O, O_ref, what=f"prefill O (S={n_splits})")
         check_close(LSE, LSE_ref, LSE_ABS, what=f"prefill LSE (S={n_splits})")
         print(f"prefill S={S} H={H}/{H_kv} T={T} d={d} splits={n_splits}: O max|d| {e_o:.2e} (norm {r_o:.2e})")
+
+
+# --------------------------------------------------------------------------- NEXT-1 token scores + top-B
+# |d| <= 1e-4 |ref| + 1e-6 * G*L_q: e is a sum of <= G*L_q fp32 exponentials (relative error ~3e-6 each: ex2.approx /
+# the degree-4 polynomial) taken against a row log-mass that is itself good to ~1e-6
+def _check_e(got, ref, rows, what):
+    g = got.double().cpu().numpy()
+    lim = 1e-4 * np.abs(ref) + 1e-6 * rows
+    worst = float((np.abs(g - ref) - lim).max())
+    assert np.isfinite(g).all() and worst <= 0, f"{what}: gate exceeded by {worst:.3e}"
+    np.testing.assert_allclose(g.sum(-1), rows, rtol=2e-5, err_msg=f"{what}: a chunk's slots must sum to G*L_q")
+
+
+TOKEN_CASES = [
+    ("tiny", dict(token_alpha=24.0)),                                           # C1
+    ("tiny", dict(C=130, N=5, K=2, keep=0.3, token_alpha=24.0)),                # full tile + 3-row tail
+    ("tiny", dict(C=200, H=8, H_kv=2, L_q=40, L_d=8, keep=0.25, token_alpha=40.0)),   # GQA: 160 scoring rows = 2 M tiles
+    ("dream16k", dict(token_gamma=3.0)),                                        # C3: 896 scoring rows = 7 M tiles
+    ("sparse32k", dict(token_gamma=4.0)),                                       # C4 at full size
+]
+
+
+@pytest.mark.parametrize("name,kw", TOKEN_CASES)
+def test_token_scores_and_topb(B, name, kw):
+    w, inp = _inputs(name, **kw)
+    shape = B.Shape.of(w)
+    dQ, dK = dev_bf16(inp["Q_dec"]), dev_bf16(inp["Kcache"])
+    e = B.score_tokens(shape, dQ, dK)
+    torch.cuda.synchronize()
+    e_ref = oracle.token_scores(inp["Q_dec"], inp["Kcache"], w.L_q)
+    _check_e(e, e_ref, w.G * w.L_q, f"token scores {name}")
+    keep = B.select_topb(shape, e)
+    torch.cuda.synchronize()
+    # the selection rule itself, decided on the same values on both sides (the GPU's fp32 scores, widened exactly)
+    check_exact(keep, oracle.topb(e.double().cpu().numpy(), w.Bk), "top-B of the GPU's scores")
+    # the planted tokens leave a clear gap (asserted on the oracle's scores), so the list is also the fp64 oracle's
+    keep_ref = oracle.topb(e_ref, w.Bk)
+    kept = np.take_along_axis(e_ref, keep_ref[..., 1:].astype(np.int64), -1).min(-1)
+    mask = np.ones(e_ref.shape, bool); np.put_along_axis(mask, keep_ref.astype(np.int64), False, -1)
+    dropped = np.where(mask, e_ref, -np.inf).max(-1)
+    # >= 1e-3 relative: a hundred times the fp32 error of a score (<= 1e-5 relative, see _check_e)
+    assert ((kept - dropped) / dropped).min() >= 1e-3, "planted-token gap too small for a bit-exact comparison"
+    check_exact(keep, keep_ref, "token_keep_idx vs the oracle")
+    check_exact(keep, inp["keep"], "planted tokens (generator sanity)")
+
+
+def test_topb_ties_nan_inf(B):
+    C, Bk = 40, 7
+    e = np.zeros((1, 1, 7, C + 1), np.float32)
+    e[0, 0, 0] = 1.0                                   # all equal: lowest slots win
+    e[0, 0, 1, 2::3] = 2.0                             # many ties above a floor
+    e[0, 0, 2] = np.nan                                # all NaN == all -inf
+    e[0, 0, 3] = -np.inf; e[0, 0, 3, [7, 30]] = 0.5    # fewer finite values than Bk - 1
+    e[0, 0, 4] = np.arange(C + 1)[::-1]; e[0, 0, 4, 5] = np.nan; e[0, 0, 4, 40] = np.inf
+    e[0, 0, 5] = np.tile([3.0, -0.0, 0.0, 1.0], 11)[: C + 1]                    # -0 ties with +0
+    e[0, 0, 6] = np.random.default_rng(0).standard_normal(C + 1); e[0, 0, 6, 0] = 100.0     # BOS kept whatever its score
+    for bk in (1, 2, Bk, C, C + 1):
+        shape = B.Shape(1, 1, 1, 128, 7, C, 1, bk, 1, 1, 1)
+        check_exact(B.select_topb(shape, dev_f32(e)), oracle.topb(e, bk), f"top-B Bk={bk}")
+
+
+@pytest.mark.parametrize("C,Bk,chunks", [(512, 129, 64), (1024, 513, 16), (2047, 100, 8), (8191, 4000, 3), (5, 3, 200)])
+def test_topb_random(B, C, Bk, chunks):
+    r = np.random.default_rng(C + Bk)
+    e = r.standard_normal((1, 1, chunks, C + 1)).astype(np.float32)
+    e[0, 0, ::2] = np.round(e[0, 0, ::2] * 4) / 4      # half of the chunks on a coarse grid: many exact ties
+    shape = B.Shape(1, 1, 1, 128, chunks, C, 1, Bk, 1, 1, 1)
+    check_exact(B.select_topb(shape, dev_f32(e)), oracle.topb(e, Bk), "top-B")
+
+
+def test_step_with_device_produced_keep_list(B):
+    """The list pdllm_select_topb writes is what pdllm_step consumes: score tokens -> top-B -> pdllm_step, against the
+    oracle run with the oracle's own list."""
+    w, inp = _inputs("tiny", C=150, H=8, H_kv=4, d=128, N=10, K=3, keep=0.4, L_q=24, L_d=40, token_alpha=40.0)
+    dev = to_device(inp)
+    shape = B.Shape.of(w)
+    keep = B.select_topb(shape, B.score_tokens(shape, dev["Q_dec"], dev["Kcache"]))
+    out = B.step(shape, dev["Q_dec"], dev["Kcache"], dev["Vcache"], keep, dev["K_dec"], dev["V_dec"], n_splits=2)
+    torch.cuda.synchronize()
+    keep_ref = oracle.topb(oracle.token_scores(inp["Q_dec"], inp["Kcache"], w.L_q), w.Bk)
+    check_exact(keep, keep_ref, "keep list")
+    ref = oracle.step(inp["Q_dec"], inp["Kcache"], inp["Vcache"], keep_ref, inp["K_dec"], inp["V_dec"], w.K, w.L_q)
+    check_exact(out["chunk_ids"], ref["ids"])
+    check_O(out["O"], ref["O"]); check_close(out["LSE"], ref["LSE"], LSE_ABS)
