@@ -45,6 +45,10 @@ class Workload:
     # every row whatever its direction: the N(0,1) configs)
     token_alpha: float = 0.0
     token_gamma: float = 1.0
+    # R8's strict reading of P:116 ("only the response tokens are processed", the query KV is cached): Q_dec holds the
+    # L_d response rows only while K_dec / V_dec hold the L_q + L_d query + response rows.  False (the BASELINE.json
+    # configs): the L_q query rows attend too, L = L_s = L_q + L_d, query rows first.
+    strict: bool = False
 
     @property
     def G(self): return self.H // self.H_kv
@@ -53,9 +57,9 @@ class Workload:
     @property
     def Bk(self): return self.Cp if self.keep >= 1.0 else 1 + int(round(self.keep * self.C))
     @property
-    def L(self): return self.L_q + self.L_d
+    def L(self): return self.L_d if self.strict else self.L_q + self.L_d
     @property
-    def L_s(self): return self.L
+    def L_s(self): return self.L_q + self.L_d
     @property
     def S_pre(self): return self.K * self.Bk
     @property
@@ -92,6 +96,12 @@ EXTRA = {
     "fig5b": Workload("fig5b", B=1, H=32, H_kv=8, d=128, N=16, C=1024, K=4, keep=1.0, L_q=16, L_d=16,
                       alpha=2.0, unit_logits=False, seed=BASE_SEED + 6),
 }
+# SURVEY 8(f) NEXT-4, the Fig. 5(b) shape as the survey wrote it: L = L_d = 32 response rows (strict R8), the cached
+# query window L_q = 64 inside K_dec / V_dec, GQA 32/8, d = 128, dense-selected KV of 8K / 16K / 32K tokens
+# (K whole chunks of C = 1024 out of a 32K prefix); the paper runs it with S = 4 splits.
+for _k, _name in ((8, "fig5b_8k"), (16, "fig5b_16k"), (32, "fig5b_32k")):
+    EXTRA[_name] = Workload(_name, B=1, H=32, H_kv=8, d=128, N=32, C=1024, K=_k, keep=1.0, L_q=64, L_d=32,
+                            alpha=2.0, unit_logits=False, seed=BASE_SEED + 7 + _k, strict=True)
 
 
 def small_variant(w: Workload, **kw) -> Workload:
@@ -144,7 +154,7 @@ def make_planted(w: Workload):
 def make_inputs(w: Workload, threads: int = 8) -> dict:
     """All tensors of one step as numpy arrays (bf16 tensors as uint16 bit patterns)."""
     sigma = 1.0 / np.sqrt(w.d) if w.unit_logits else 1.0
-    Q = f32_to_bf16_bits(_normal(w.seed, T_Q, 0, (w.B, w.H, w.L, w.d), sigma))
+    Q = f32_to_bf16_bits(_normal(w.seed, T_Q, 0, (w.B, w.H, w.L_q + w.L_d, w.d), sigma))     # query rows, then response rows
     Kd = f32_to_bf16_bits(_normal(w.seed, T_KD, 0, (w.B, w.H_kv, w.L_s, w.d), sigma))
     Vd = f32_to_bf16_bits(_normal(w.seed, T_VD, 0, (w.B, w.H_kv, w.L_s, w.d), sigma))
     keep = make_keep(w)
@@ -173,4 +183,6 @@ def make_inputs(w: Workload, threads: int = 8) -> dict:
     else:
         for bg in range(n):
             slab(bg)
-    return dict(Q_dec=Q, Kcache=Kc, Vcache=Vc, K_dec=Kd, V_dec=Vd, keep=keep, planted=planted)
+    Q_score = np.ascontiguousarray(Q[:, :, : w.L_q])                # the scoring rows (the query window)
+    Q_dec = np.ascontiguousarray(Q[:, :, w.L_q:]) if w.strict else Q
+    return dict(Q_dec=Q_dec, Q_score=Q_score, Kcache=Kc, Vcache=Vc, K_dec=Kd, V_dec=Vd, keep=keep, planted=planted)

@@ -214,3 +214,38 @@ def test_step_with_device_produced_keep_list(B):
     ref = oracle.step(inp["Q_dec"], inp["Kcache"], inp["Vcache"], keep_ref, inp["K_dec"], inp["V_dec"], w.K, w.L_q)
     check_exact(out["chunk_ids"], ref["ids"])
     check_O(out["O"], ref["O"]); check_close(out["LSE"], ref["LSE"], LSE_ABS)
+
+
+# --------------------------------------------------------------------------- NEXT-4 the paper's Fig. 5(b) decode shapes
+@pytest.mark.parametrize("name", ["fig5b_8k", "fig5b_16k", "fig5b_32k"])
+def test_fig5b_strict_decode_shapes_full_size(B, name):
+    """P:189-193 / Fig. 5(b): L = L_d = 32 response rows per head (R8 strict: the cached query rows sit in K_dec /
+    V_dec, L_s = L_q + L_d = 96), GQA 32/8 (one packed 128-row query tile per KV head), dense-selected KV of 8K-32K
+    tokens: the static-selection flow -- scores and top-K from the query window, then attention with the paper's
+    S = 4 and the automatic split count, through the gather path and through the compact cache (TMA tiles)."""
+    w = W.EXTRA[name]
+    inp = W.make_inputs(w)
+    dev = to_device(inp)
+    shape = B.Shape.of(w)
+    assert (shape.L, shape.L_s, shape.H // shape.H_kv * shape.L) == (32, 96, 128)
+    sc = B.score_chunks(shape, dev_bf16(inp["Q_score"]), dev["Kcache"])
+    ids = B.select_topk(shape, sc)
+    torch.cuda.synchronize()
+    sc_ref = oracle.scores(inp["Q_score"], inp["Kcache"], w.L_q)
+    check_close(sc, sc_ref, SCORE_ABS, what="scores")
+    ids_ref = oracle.topk(sc_ref, w.K)
+    check_exact(ids, ids_ref, "chunk ids")
+    O_ref, LSE_ref = oracle.attn(inp["Q_dec"], inp["Kcache"], inp["Vcache"], ids_ref, None, inp["K_dec"], inp["V_dec"])
+    for S in (0, 4):
+        O, LSE = B.sparse_attn(shape, dev["Q_dec"], dev["Kcache"], dev["Vcache"], ids, None, dev["K_dec"], dev["V_dec"], n_splits=S)
+        torch.cuda.synchronize()
+        e_o, r_o = check_O(O, O_ref, what=f"O (S={S})")
+        check_close(LSE, LSE_ref, LSE_ABS, what=f"LSE (S={S})")
+        print(f"{name} gather S={S} (auto={B.auto_splits(shape, B.num_sms())}): O max|d| {e_o:.2e} (norm {r_o:.2e})")
+    Kc, Vc = B.compact_kv(shape, dev["Kcache"], dev["Vcache"], ids, None)
+    ds = B.DenseShape.static_of(shape)
+    for S in (0, 4):
+        O, LSE = B.static_attn(ds, dev["Q_dec"], Kc, Vc, dev["K_dec"], dev["V_dec"], n_splits=S)
+        torch.cuda.synchronize()
+        check_O(O, O_ref, what=f"static O (S={S})")
+        check_close(LSE, LSE_ref, LSE_ABS, what=f"static LSE (S={S})")
