@@ -462,6 +462,295 @@ def run_ours(args, w):
         dist.destroy_process_group()
 
 
+# --------------------------------------------------------------------------- the rows after the hot path
+def _common_setup(args):
+    import torch
+    from paper_2606_10537_b200 import binding as B
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the pdllm hot path has no CPU fallback")
+    torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+    B.lib()
+    return torch, B
+
+
+def _timed(torch, fn, K, flush_buf=None):
+    """us per call over K calls on the current stream (per-call events with an L2 flush between calls when asked)."""
+    if flush_buf is None:
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        for _ in range(K):
+            fn()
+        b.record()
+        torch.cuda.synchronize()
+        return 1e3 * a.elapsed_time(b) / K
+    pairs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
+    for a, b in pairs:
+        flush_buf.zero_()
+        a.record()
+        fn()
+        b.record()
+    torch.cuda.synchronize()
+    return 1e3 * sum(a.elapsed_time(b) for a, b in pairs) / K
+
+
+def _timed_graph(torch, fn, K):
+    """us per call of fn replayed as a CUDA graph (for stages of a few microseconds, where the host's launch rate and
+    not the device would otherwise be what is timed)."""
+    g = torch.cuda.CUDAGraph()
+    cs = torch.cuda.Stream()
+    cs.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(cs):
+        fn()
+        cs.synchronize()
+        with torch.cuda.graph(g, stream=cs):
+            fn()
+    torch.cuda.current_stream().wait_stream(cs)
+    for _ in range(3):
+        g.replay()
+    return _timed(torch, g.replay, K)
+
+
+def _attn_roofline(peaks, flops, nbytes, us, kernel):
+    t_tensor, t_hbm = flops / (peaks["bf16_tflops_sustained"] * 1e12), nbytes / (peaks["hbm_gbs"] * 1e9)
+    t_spec = max(flops / (SPEC_PEAKS["bf16_tflops"] * 1e12), nbytes / (SPEC_PEAKS["hbm_gbs"] * 1e9))
+    bound = "tensor" if t_tensor >= t_hbm else "hbm"
+    tf, gbs = flops / (us * 1e-6) / 1e12, nbytes / (us * 1e-6) / 1e9
+    return {"kernel": kernel, "bound": bound, "achieved": tf if bound == "tensor" else gbs,
+            "peak": peaks["bf16_tflops_sustained"] if bound == "tensor" else peaks["hbm_gbs"],
+            "unit": "TFLOP/s" if bound == "tensor" else "GB/s", "frac": max(t_tensor, t_hbm) / (us * 1e-6),
+            "frac_of_spec_peak": t_spec / (us * 1e-6), "peak_source": peaks["source"], "traffic": None, "us": us,
+            "tflops": tf, "gbs": gbs, "roofline_us": 1e6 * max(t_tensor, t_hbm)}
+
+
+def _line(args, w, value, config, roofline, cpu, e2e, launches, clocks, extra):
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": 1, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": value / 1e3, "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
+            "data": "synthetic", "config": config, "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e,
+            "gpu_launches": launches, "clocks": clocks}
+    line.update(extra)
+    print(json.dumps(line))
+
+
+def run_static(args, w):
+    """--mode static: the paper's static-selection mode -- per step only the attention, through the gather
+    path (pdllm_sparse_attn) and through the compact cache (pdllm_compact_kv once, then pdllm_static_attn: TMA tiles);
+    beside it the per-step re-selection cost with the pooled-key scorer (pdllm_score_chunks_pooled + pdllm_select_topk)
+    against the full chunk-score kernel."""
+    torch, B = _common_setup(args)
+    shape = B.Shape.of(w)
+    inp = W.make_inputs(w)
+    bf = lambda bits: torch.from_numpy(np.ascontiguousarray(bits).view(np.int16)).cuda().view(torch.bfloat16)
+    dQ, dQs, dKc, dVc, dKd, dVd = (bf(inp[k]) for k in ("Q_dec", "Q_score", "Kcache", "Vcache", "K_dec", "V_dec"))
+    dkeep = None if inp["keep"] is None else torch.from_numpy(inp["keep"]).cuda()
+    K, Wm = args.steps, args.warmup
+    flush = torch.empty((256 << 20,), dtype=torch.uint8, device="cuda") if needs_flush(w) else None
+    sc = B.score_chunks(shape, dQs, dKc)
+    ids = B.select_topk(shape, sc)
+    kbar = B.pool_keys(shape, dKc)
+    sc_p = B.score_chunks_pooled(shape, dQs, kbar)
+    ids_p = B.select_topk(shape, sc_p)
+    torch.cuda.synchronize()
+    recall = float(np.mean([len(set(a) & set(b)) / w.K for a, b in zip(ids_p.cpu().numpy().reshape(-1, w.K), inp["planted"].reshape(-1, w.K))]))
+    ids_ok = bool((ids.cpu().numpy() == inp["planted"]).all())
+    Kc, Vc = B.compact_kv(shape, dKc, dVc, ids, dkeep)
+    ds = B.DenseShape.static_of(shape)
+    S = args.n_splits if args.n_splits > 0 else B.auto_splits(shape, B.num_sms())
+    Sd = args.n_splits if args.n_splits > 0 else B.dense_auto_splits(ds, B.num_sms())
+    ws, wsd = B.alloc_workspace(shape, args.n_splits), B.alloc_dense_workspace(ds, args.n_splits)
+    O = torch.empty((w.B, w.H, w.L, w.d), dtype=torch.bfloat16, device="cuda")
+    LSE = torch.empty((w.B, w.H, w.L), dtype=torch.float32, device="cuda")
+    gather = lambda: B.sparse_attn(shape, dQ, dKc, dVc, ids, dkeep, dKd, dVd, n_splits=args.n_splits, O=O, LSE=LSE, workspace=ws)
+    static = lambda: B.static_attn(ds, dQ, Kc, Vc, dKd, dVd, n_splits=args.n_splits, O=O, LSE=LSE, workspace=wsd)
+    pooled = lambda: B.select_topk(shape, B.score_chunks_pooled(shape, dQs, kbar, scores=sc_p), chunk_ids=ids_p)
+    full = lambda: B.select_topk(shape, B.score_chunks(shape, dQs, dKc, scores=sc), chunk_ids=ids)
+    for _ in range(Wm):
+        gather(); static(); pooled()
+    torch.cuda.synchronize()
+    with ClockSampler(0) as clk:
+        us_static = _timed(torch, static, K, flush)
+        us_gather = _timed(torch, gather, K, flush)
+    us_pooled = _timed_graph(torch, pooled, K)
+    us_full = _timed_graph(torch, full, max(3, K // 10))
+    us_compact = _timed(torch, lambda: B.compact_kv(shape, dKc, dVc, ids, dkeep, Kc, Vc), max(3, K // 10))
+    us_pool = _timed(torch, lambda: B.pool_keys(shape, dKc, kbar), max(3, K // 10))
+    # e2e: the per-step tensors come from pinned host memory and O goes back, around the C-ABI call
+    pin = lambda bits: torch.from_numpy(np.ascontiguousarray(bits).view(np.int16)).view(torch.bfloat16).pin_memory()
+    hQ, hK, hV = pin(inp["Q_dec"]), pin(inp["K_dec"]), pin(inp["V_dec"])
+    hO = torch.empty(O.shape, dtype=torch.bfloat16).pin_memory()
+
+    def host_step():
+        dQ.copy_(hQ, non_blocking=True); dKd.copy_(hK, non_blocking=True); dVd.copy_(hV, non_blocking=True)
+        static()
+        hO.copy_(O, non_blocking=True)
+        torch.cuda.current_stream().synchronize()
+    for _ in range(Wm):
+        host_step()
+    t0 = time.perf_counter()
+    for _ in range(K):
+        host_step()
+    e2e_us = 1e6 * (time.perf_counter() - t0) / K
+    peaks = load_peaks()
+    roof = _attn_roofline(peaks, w.attn_flops(), w.attn_bytes(), us_static,
+                          "attn_kernel, contiguous mode (3-D TMA tiles)" + (" + combine_kernel" if Sd > 1 else ""))
+    roof_g = _attn_roofline(peaks, w.attn_flops(), w.attn_bytes(), us_gather,
+                            "attn_kernel, gather mode (cp.async)" + (" + combine_kernel" if S > 1 else ""))
+    from oracle import oracle
+    cores = oracle.num_threads()
+    n = max(1, min(w.H_kv, cores // max(1, min(w.G, cores))))
+    sl = {k: np.ascontiguousarray(inp[k][:1, : (n * w.G if k == "Q_dec" else n)]) for k in ("Q_dec", "Kcache", "Vcache", "K_dec", "V_dec")}
+    kp = None if inp["keep"] is None else np.ascontiguousarray(inp["keep"][:1, :n])
+    t0 = time.perf_counter()
+    oracle.attn(sl["Q_dec"], sl["Kcache"], sl["Vcache"], np.ascontiguousarray(inp["planted"][:1, :n]), kp, sl["K_dec"], sl["V_dec"])
+    t_or = time.perf_counter() - t0
+    factor = w.B * w.H_kv / n
+    cpu = {"value": 1e6 * t_or * factor, "unit": UNIT, "cores": cores, "kind": "oracle",
+           "sample": f"attention of {n} of {w.B * w.H_kv} (batch, KV-head) groups, time scaled x{factor:g}"}
+    cfg = workload_config(w, Sd)
+    cfg.update(mode="static", call="pdllm_static_attn over the compact cache of pdllm_compact_kv (static selection, P:116)",
+               n_splits_gather=S)
+    _line(args, w, us_static, cfg, roof, cpu,
+          {"value": e2e_us, "unit": UNIT, "h2d_bytes_per_step": hQ.numel() * 2 + hK.numel() * 2 + hV.numel() * 2,
+           "d2h_bytes_per_step": hO.numel() * 2, "call": "pinned host Q_dec/K_dec/V_dec in, O out, around pdllm_static_attn"},
+          K * (1 + (1 if Sd > 1 else 0)), clk.summary(),
+          {"static_mode_us": {"static_attn_tma_tiles": us_static, "sparse_attn_gather": us_gather,
+                              "reselect_pooled_scorer_plus_topk": us_pooled, "reselect_full_scorer_plus_topk": us_full,
+                              "compact_kv_once": us_compact, "pool_keys_once": us_pool},
+           "roofline_gather": roof_g, "pooled_scorer_recall_of_planted_chunks": recall, "full_scorer_ids_ok": ids_ok})
+
+
+def run_tokens(args, w):
+    """--mode tokens: NEXT-1 on the workload's shape with planted tokens: pdllm_score_tokens (two streaming passes over
+    the K cache) and pdllm_select_topb; HBM roofline of the pair of passes."""
+    torch, B = _common_setup(args)
+    if w.keep >= 1.0:
+        w = W.small_variant(w, keep=0.5)
+    w = W.small_variant(w, token_gamma=4.0) if not w.unit_logits else W.small_variant(w, token_alpha=24.0)
+    shape = B.Shape.of(w)
+    inp = W.make_inputs(w)
+    bf = lambda bits: torch.from_numpy(np.ascontiguousarray(bits).view(np.int16)).cuda().view(torch.bfloat16)
+    dQs, dKc = bf(inp["Q_score"]), bf(inp["Kcache"])
+    e = torch.empty((w.B, w.H_kv, w.N, w.Cp), dtype=torch.float32, device="cuda")
+    keep = torch.empty((w.B, w.H_kv, w.N, w.Bk), dtype=torch.int32, device="cuda")
+    ws = torch.empty((B.lib().pdllm_score_tokens_workspace_bytes(__import__("ctypes").byref(shape.c())),), dtype=torch.uint8, device="cuda")
+    sc = torch.empty((w.B, w.H_kv, w.N), dtype=torch.float32, device="cuda")
+    K, Wm = args.steps, args.warmup
+    flush = torch.empty((256 << 20,), dtype=torch.uint8, device="cuda") if needs_flush(w) else None
+    tok = lambda: B.score_tokens(shape, dQs, dKc, token_scores=e, workspace=ws)
+    for _ in range(Wm):
+        tok(); B.select_topb(shape, e, keep)
+    torch.cuda.synchronize()
+    ok = bool((keep.cpu().numpy() == inp["keep"]).all())
+    with ClockSampler(0) as clk:
+        us_tok = _timed(torch, tok, K, flush)
+    us_pass1 = _timed(torch, lambda: B.score_chunks(shape, dQs, dKc, scores=sc), K, flush)
+    us_topb = _timed_graph(torch, lambda: B.select_topb(shape, e, keep), K)
+    rows = w.G * w.L_q
+    nbytes = 2 * w.B * w.H_kv * w.N * w.Cp * w.d * 2 + 2 * w.B * w.H * w.L_q * w.d * 2 \
+        + 2 * 4 * w.B * w.H_kv * w.N * rows + 4 * w.B * w.H_kv * w.N * w.Cp
+    peaks = load_peaks()
+    flops = 2 * w.score_flops()           # Q K^T once per pass
+    roof = _attn_roofline(peaks, flops, nbytes, us_tok, "score_kernel (row log-masses) + token_score_kernel (NEXT-1)")
+    roof["algorithmic_bytes"] = nbytes
+    roof["token_score_kernel_alone"] = _attn_roofline(peaks, flops / 2, nbytes / 2, max(us_tok - us_pass1, 1e-3), "token_score_kernel")
+    from oracle import oracle
+    cores = oracle.num_threads()
+    n = max(1, min(w.H_kv, cores))
+    nch = max(1, min(w.N, 4))
+    t0 = time.perf_counter()
+    oracle.token_scores(np.ascontiguousarray(inp["Q_score"][:1, : n * w.G]), np.ascontiguousarray(inp["Kcache"][:1, :n, :nch]), w.L_q)
+    t_or = time.perf_counter() - t0
+    factor = (w.B * w.H_kv / n) * (w.N / nch)
+    cpu = {"value": 1e6 * t_or * factor, "unit": UNIT, "cores": cores, "kind": "oracle",
+           "sample": f"token scores of {nch} of {w.N} chunks of {n} of {w.B * w.H_kv} groups, time scaled x{factor:g}"}
+    hQ = torch.from_numpy(np.ascontiguousarray(inp["Q_score"]).view(np.int16)).view(torch.bfloat16).pin_memory()
+    hkeep = torch.empty(keep.shape, dtype=torch.int32).pin_memory()
+
+    def host_step():
+        dQs.copy_(hQ, non_blocking=True)
+        tok(); B.select_topb(shape, e, keep)
+        hkeep.copy_(keep, non_blocking=True)
+        torch.cuda.current_stream().synchronize()
+    for _ in range(Wm):
+        host_step()
+    t0 = time.perf_counter()
+    for _ in range(K):
+        host_step()
+    e2e_us = 1e6 * (time.perf_counter() - t0) / K
+    cfg = workload_config(w, None)
+    cfg.update(mode="tokens", call="pdllm_score_tokens (+ pdllm_select_topb): Eq. 5 query->chunk eviction scores, top-B retention",
+               token_planting={"token_alpha": w.token_alpha, "token_gamma": w.token_gamma})
+    _line(args, w, us_tok + us_topb, cfg, roof, cpu,
+          {"value": e2e_us, "unit": UNIT, "h2d_bytes_per_step": hQ.numel() * 2, "d2h_bytes_per_step": hkeep.numel() * 4,
+           "call": "pinned host query window in, token_keep_idx out, around pdllm_score_tokens + pdllm_select_topb"},
+          K * (3 + (1 if rows > 128 else 0)), clk.summary(),
+          {"tokens_mode_us": {"score_tokens_two_passes": us_tok, "of_which_chunk_score_pass": us_pass1, "select_topb": us_topb},
+           "planted_tokens_recovered": ok})
+
+
+def run_prefill(args, w):
+    """--mode prefill: NEXT-2, the attention of the chunk prefill on the workload's prefix: N sequences [BOS; c_i; q; m]
+    (|m| = 16 pseudo-labels) per batch element, all heads; tensor roofline."""
+    torch, B = _common_setup(args)
+    T = w.Cp + w.L_q + 16
+    S = w.B * w.N
+    r = np.random.Generator(np.random.Philox(key=[(w.seed << 8) + 9, 0]))
+    mk = lambda shp: torch.from_numpy(W.f32_to_bf16_bits(r.standard_normal(shp, dtype=np.float32)).view(np.int16)).view(torch.bfloat16)
+    hQ, hK, hV = mk((S, w.H, T, w.d)).pin_memory(), mk((S, w.H_kv, T, w.d)).pin_memory(), mk((S, w.H_kv, T, w.d)).pin_memory()
+    dQ, dK, dV = hQ.cuda(), hK.cuda(), hV.cuda()
+    ds = B.DenseShape(S, w.H, w.H_kv, w.d, T, T, 0)
+    Sd = args.n_splits if args.n_splits > 0 else B.dense_auto_splits(ds, B.num_sms())
+    ws = B.alloc_dense_workspace(ds, args.n_splits)
+    O = torch.empty((S, w.H, T, w.d), dtype=torch.bfloat16, device="cuda")
+    LSE = torch.empty((S, w.H, T), dtype=torch.float32, device="cuda")
+    K, Wm = args.steps, args.warmup
+    fn = lambda: B.prefill_attn(ds, dQ, dK, dV, n_splits=args.n_splits, O=O, LSE=LSE, workspace=ws)
+    for _ in range(Wm):
+        fn()
+    torch.cuda.synchronize()
+    kv_bytes = 2 * S * w.H_kv * T * w.d * 2
+    flush = torch.empty((256 << 20,), dtype=torch.uint8, device="cuda") if kv_bytes < 4 * L2_BYTES else None
+    with ClockSampler(0) as clk:
+        us = _timed(torch, fn, K, flush)
+    flops = 4.0 * S * w.H * T * T * w.d
+    nbytes = kv_bytes + 2 * S * w.H * T * w.d * 2 + 4 * S * w.H * T
+    roof = _attn_roofline(load_peaks(), flops, nbytes, us, "attn_kernel, contiguous mode (chunk prefill)" + (" + combine_kernel" if Sd > 1 else ""))
+    from oracle import oracle
+    cores = oracle.num_threads()
+    nh = max(1, min(w.H_kv, cores // max(1, w.G)))
+    Tq = min(T, 256)                      # a bounded sample: the first Tq query rows of nh KV heads of one sequence
+    q = np.ascontiguousarray(hQ.view(torch.int16).numpy().view(np.uint16)[:1, : nh * w.G])
+    k = np.ascontiguousarray(hK.view(torch.int16).numpy().view(np.uint16)[:1, :nh])
+    v = np.ascontiguousarray(hV.view(torch.int16).numpy().view(np.uint16)[:1, :nh])
+    t0 = time.perf_counter()
+    oracle.prefill_attn(q, k, v)
+    t_or = time.perf_counter() - t0
+    factor = S * w.H_kv / nh
+    cpu = {"value": 1e6 * t_or * factor, "unit": UNIT, "cores": cores, "kind": "oracle",
+           "sample": f"one sequence, {nh} of {w.H_kv} KV heads (all {T} rows), time scaled x{factor:g}"}
+    hO = torch.empty(O.shape, dtype=torch.bfloat16).pin_memory()
+
+    def host_step():
+        dQ.copy_(hQ, non_blocking=True); dK.copy_(hK, non_blocking=True); dV.copy_(hV, non_blocking=True)
+        fn()
+        hO.copy_(O, non_blocking=True)
+        torch.cuda.current_stream().synchronize()
+    for _ in range(min(Wm, 3)):
+        host_step()
+    Ke = max(3, K // 10)
+    t0 = time.perf_counter()
+    for _ in range(Ke):
+        host_step()
+    e2e_us = 1e6 * (time.perf_counter() - t0) / Ke
+    cfg = {"workload": f"chunk prefill of '{w.name}': {S} sequences [BOS; c_i; q; m] of T = {T} rows (C = {w.C}, L_q = {w.L_q}, |m| = 16)",
+           "mode": "prefill", "S": S, "H": w.H, "H_kv": w.H_kv, "d": w.d, "T": T, "n_splits": Sd,
+           "call": "pdllm_prefill_attn (Eq. 2; SURVEY 8(f) NEXT-2)",
+           "l2": "explicit 256 MB flush between iterations" if flush is not None else "K/V larger than L2, no explicit flush"}
+    _line(args, w, us, cfg, roof, cpu,
+          {"value": e2e_us, "unit": UNIT, "h2d_bytes_per_step": (hQ.numel() + hK.numel() + hV.numel()) * 2,
+           "d2h_bytes_per_step": hO.numel() * 2, "call": "pinned host Q/K/V in, O out, around pdllm_prefill_attn"},
+          K * (1 + (1 if Sd > 1 else 0)), clk.summary(), {})
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -470,6 +759,9 @@ def main():
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--workload", choices=list(W.CONFIGS) + list(W.EXTRA), default="sparse32k")
     ap.add_argument("--n-splits", type=int, default=0, help="0 = pdllm_auto_splits")
+    ap.add_argument("--mode", choices=["step", "static", "tokens", "prefill"], default="step",
+                    help="step: pdllm_step (the metric's per-step call, default); static / tokens / prefill: the rows "
+                         "after the hot path (SURVEY 8(f)), 1 GPU")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "ours" and args.gpus > 1 and int(os.environ.get("WORLD_SIZE", "1")) != args.gpus:
@@ -479,6 +771,14 @@ def main():
     w = W.CONFIGS[args.workload] if args.workload in W.CONFIGS else W.EXTRA[args.workload]
     if args.impl == "reference":
         run_reference(args, w)
+    elif args.mode == "static":
+        run_static(args, w)
+    elif args.mode == "tokens":
+        run_tokens(args, w)
+    elif args.mode == "prefill":
+        run_prefill(args, w)
+    elif w.strict:
+        raise SystemExit(f"bench.py: workload {w.name} has no query rows in Q_dec (strict R8 rows): use --mode static")
     else:
         run_ours(args, w)
 

@@ -61,26 +61,30 @@ __global__ void __launch_bounds__(256) pool_keys_kernel(const uint16_t *__restri
     }
 }
 
-// One CTA per (b,g): qbar = mean of the G*L_q scoring rows (fixed summation order), then one warp per chunk:
-// scores[n] = log(C+1) + scale * <qbar, kbar[n]>.
+// One CTA per (b,g): qbar = mean of the G*L_q scoring rows (16-byte loads, the row slots' partial sums meet in shared
+// memory in a fixed order), then one warp per chunk: scores[n] = log(C+1) + scale * <qbar, kbar[n]>.
 template <int D>
-__global__ void __launch_bounds__(256) pooled_score_kernel(const uint16_t *__restrict__ Q, int64_t q_batch_stride,
+__global__ void __launch_bounds__(512) pooled_score_kernel(const uint16_t *__restrict__ Q, int64_t q_batch_stride,
                                                            int64_t q_head_stride, const float *__restrict__ kbar,
                                                            float *__restrict__ scores, int H_kv, int G, int N, int L_q,
                                                            float scale, float log_cp) {
-    constexpr int kSlots = 256 / D;                           // row slots: 2 (d = 128) or 4 (d = 64)
+    constexpr int kLanesPerRow = D / 8;
+    constexpr int kSlots = 512 / kLanesPerRow;                // row slots: 32 (d = 128) or 64 (d = 64)
     __shared__ float part[kSlots][D];
     __shared__ float qbar[D];
     const int bg = blockIdx.x, b = bg / H_kv, g = bg % H_kv;
-    const int c = threadIdx.x % D, rs = threadIdx.x / D;
+    const int c8 = threadIdx.x % kLanesPerRow, rs = threadIdx.x / kLanesPerRow;
     const int rows = G * L_q;
-    float acc = 0.f;
+    float acc[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
     for (int m = rs; m < rows; m += kSlots) {
         const int hh = m / L_q, i = m - hh * L_q;
-        const uint16_t v = Q[(int64_t)b * q_batch_stride + (int64_t)(g * G + hh) * q_head_stride + (int64_t)i * D + c];
-        acc += __uint_as_float((uint32_t)v << 16);
+        const uint4 u = __ldg(reinterpret_cast<const uint4 *>(Q + (int64_t)b * q_batch_stride +
+                                                              (int64_t)(g * G + hh) * q_head_stride + (int64_t)i * D + c8 * 8));
+        acc[0] += bf16_lo(u.x); acc[1] += bf16_hi(u.x); acc[2] += bf16_lo(u.y); acc[3] += bf16_hi(u.y);
+        acc[4] += bf16_lo(u.z); acc[5] += bf16_hi(u.z); acc[6] += bf16_lo(u.w); acc[7] += bf16_hi(u.w);
     }
-    part[rs][c] = acc;
+#pragma unroll
+    for (int e = 0; e < 8; ++e) part[rs][c8 * 8 + e] = acc[e];
     __syncthreads();
     if (threadIdx.x < D) {
         float s = 0.f;
@@ -89,7 +93,7 @@ __global__ void __launch_bounds__(256) pooled_score_kernel(const uint16_t *__res
     }
     __syncthreads();
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    for (int n = warp; n < N; n += 8) {
+    for (int n = warp; n < N; n += 16) {
         const float *kb = kbar + ((int64_t)bg * N + n) * D;
         float s = 0.f;
         for (int e = lane; e < D; e += 32) s += qbar[e] * kb[e];
@@ -125,10 +129,10 @@ cudaError_t launch_pooled_scores(const Dims &s, const void *Q, int64_t q_batch_s
     const unsigned groups = (unsigned)(s.B * s.H_kv);
     const float log_cp = logf((float)s.Cp);
     if (s.d == 128)
-        pooled_score_kernel<128><<<groups, 256, 0, st>>>(static_cast<const uint16_t *>(Q), q_batch_stride, q_head_stride, kbar,
+        pooled_score_kernel<128><<<groups, 512, 0, st>>>(static_cast<const uint16_t *>(Q), q_batch_stride, q_head_stride, kbar,
                                                          scores, s.H_kv, s.G, s.N, s.L_q, s.scale, log_cp);
     else
-        pooled_score_kernel<64><<<groups, 256, 0, st>>>(static_cast<const uint16_t *>(Q), q_batch_stride, q_head_stride, kbar,
+        pooled_score_kernel<64><<<groups, 512, 0, st>>>(static_cast<const uint16_t *>(Q), q_batch_stride, q_head_stride, kbar,
                                                         scores, s.H_kv, s.G, s.N, s.L_q, s.scale, log_cp);
     return cudaGetLastError();
 }

@@ -305,14 +305,34 @@ __global__ void __launch_bounds__(kTopbThreads) topb_kernel(const float *__restr
             if ((k & mask) == prefix) atomicAdd(&s_hist[(k >> shift) & 0xffu], 1);
         }
         __syncthreads();
-        if (tid == 0) {
-            int need = s_need, d = 255;
-            for (; d > 0; --d) {
-                if (s_hist[d] >= need) break;
-                need -= s_hist[d];
+        if (tid < 32) {
+            // warp 0 walks the 256 bins from the top: lane l owns bins 255 - 8l .. 248 - 8l; a suffix scan over the
+            // lanes finds the lane in whose bins the need-th largest key falls, which then walks its eight bins
+            const int need = s_need;
+            int h[8], mine = 0;
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                h[i] = s_hist[255 - 8 * tid - i];
+                mine += h[i];
             }
-            s_prefix = prefix | ((uint32_t)d << shift);
-            s_need = need;                    // how many keys equal to the final threshold are taken (lowest slots first)
+            int incl = mine;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int t = __shfl_up_sync(0xffffffffu, incl, o);
+                if (tid >= o) incl += t;
+            }
+            const int before = incl - mine;                   // keys in the bins above this lane's
+            if (before < need && need <= incl) {
+                int left = need - before, d = 255 - 8 * tid;
+#pragma unroll
+                for (int i = 0; i < 8; ++i) {
+                    if (h[i] >= left) break;
+                    left -= h[i];
+                    --d;
+                }
+                s_prefix = prefix | ((uint32_t)d << shift);
+                s_need = left;                // how many keys equal to the final threshold are taken (lowest slots first)
+            }
         }
         __syncthreads();
     }
