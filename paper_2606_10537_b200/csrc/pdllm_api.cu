@@ -104,11 +104,17 @@ int effective_splits(const Dims &d, int n_splits, int num_sms) {
 // scratch of the attention: 256 bytes for the work-item counter of the persistent kernel (always), then, for S > 1,
 // the fp32 partials O_part [S, rows, d] and lse_part [S, rows]
 constexpr size_t kCounterBytes = 256;
-size_t workspace_for(const Dims &d, int S) {
-    if (S <= 1) return kCounterBytes;
-    const size_t rows = (size_t)d.B * d.H * d.L;
-    return kCounterBytes + align_up((size_t)S * rows * d.d * sizeof(float), 256) + align_up((size_t)S * rows * sizeof(float), 256);
+// (pdllm_step only) per-M-tile chunk-score partials when G*L_q > 128: summed in a fixed order by the top-K kernel
+size_t score_partial_bytes(const Dims &d) {
+    const size_t m_tiles = ((size_t)d.G * d.L_q + kTileM - 1) / kTileM;
+    return m_tiles > 1 ? align_up(m_tiles * d.B * d.H_kv * d.N * sizeof(float), 256) : 0;
 }
+size_t partials_bytes(const Dims &d, int S) {
+    if (S <= 1) return 0;
+    const size_t rows = (size_t)d.B * d.H * d.L;
+    return align_up((size_t)S * rows * d.d * sizeof(float), 256) + align_up((size_t)S * rows * sizeof(float), 256);
+}
+size_t workspace_for(const Dims &d, int S) { return kCounterBytes + partials_bytes(d, S) + score_partial_bytes(d); }
 
 struct HostScratch {
     size_t q, kd, vd, scores, ids, o, lse, ws, total;
@@ -201,7 +207,7 @@ int pdllm_score_chunks(const pdllm_shape *shape, const void *Q, int64_t q_batch_
     if (int rc = resolve(&sh, false, &d)) return rc;
     if (!aligned16(Q) || !aligned16(Kcache) || !aligned16(scores)) return PDLLM_ERR_ALIGN;
     if ((q_batch_stride & 7) || (q_head_stride & 7) || q_head_stride < (int64_t)d.L_q * d.d) return PDLLM_ERR_ALIGN;
-    return cuda_rc(launch_score(d, Q, q_batch_stride, q_head_stride, Kcache, scores, nullptr, static_cast<cudaStream_t>(stream)));
+    return cuda_rc(launch_score(d, Q, q_batch_stride, q_head_stride, Kcache, scores, nullptr, nullptr, static_cast<cudaStream_t>(stream)));
 }
 
 int pdllm_select_topk(const pdllm_shape *shape, const float *scores, int32_t *chunk_ids, pdllm_stream_t stream) {
@@ -419,7 +425,7 @@ int pdllm_score_tokens(const pdllm_shape *shape, const void *Q, int64_t q_batch_
     float *row_lse = reinterpret_cast<float *>(base + t.row_lse);
     // pass 1: the chunk-score kernel exports every scoring row's log-mass per chunk; pass 2: the token kernel
     if (int rc = cuda_rc(launch_score(d, Q, q_batch_stride, q_head_stride, Kcache, reinterpret_cast<float *>(base + t.scores),
-                                      row_lse, st)))
+                                      row_lse, nullptr, st)))
         return rc;
     return cuda_rc(launch_token_scores(d, Q, q_batch_stride, q_head_stride, Kcache, row_lse, token_scores,
                                        reinterpret_cast<float *>(base + t.part), st));
@@ -472,10 +478,14 @@ int pdllm_step_profiled(const pdllm_shape *shape, const void *Q_dec, const void 
     // the attention's work-item counter is cleared here, far ahead of its kernel (off the step's critical path)
     if (int rc = cuda_rc(cudaMemsetAsync(workspace, 0, sizeof(int32_t), st))) return rc;
     if (int rc = record(ev ? ev->begin : nullptr, st)) return rc;
-    if (int rc = cuda_rc(launch_score(d, Q_dec, (int64_t)d.H * d.L * d.d, (int64_t)d.L * d.d, Kcache, scores_out, nullptr, st)))
+    // with several M tiles of scoring rows (G*L_q > 128) the score kernel leaves per-M-tile partials in the workspace
+    // and the top-K kernel sums them in M-tile order: no float atomics, bit-reproducible scores
+    float *sp = score_partial_bytes(d) ? reinterpret_cast<float *>(static_cast<char *>(workspace) + kCounterBytes + partials_bytes(d, S))
+                                       : nullptr;
+    if (int rc = cuda_rc(launch_score(d, Q_dec, (int64_t)d.H * d.L * d.d, (int64_t)d.L * d.d, Kcache, scores_out, nullptr, sp, st)))
         return rc;
     if (int rc = record(ev ? ev->after_score : nullptr, st)) return rc;
-    if (int rc = cuda_rc(launch_topk(d, scores_out, chunk_ids_out, st))) return rc;
+    if (int rc = cuda_rc(launch_topk(d, scores_out, chunk_ids_out, st, sp, scores_out))) return rc;
     if (int rc = record(ev ? ev->after_topk : nullptr, st)) return rc;
     return attn_impl(d, Q_dec, Kcache, Vcache, chunk_ids_out, token_keep_idx, K_dec, V_dec, S, O, LSE, gather_idx_out,
                      workspace, true, ev ? ev->after_attn : nullptr, ev ? ev->end : nullptr, st);
@@ -531,9 +541,10 @@ int pdllm_step_host(const pdllm_shape *shape, const void *h_Q_dec, const void *h
     if (cudaMemcpyAsync(base + h.vd, h_V_dec, kb, cudaMemcpyHostToDevice, st2) != cudaSuccess) return PDLLM_ERR_CUDA;
     if (side && cudaEventRecord(ev_join, st2) != cudaSuccess) return PDLLM_ERR_CUDA;
     if (int rc = cuda_rc(cudaMemsetAsync(base + h.ws, 0, sizeof(int32_t), st))) return rc;
-    if (int rc = cuda_rc(launch_score(dv, base + h.q, (int64_t)dv.H * dv.L * dv.d, (int64_t)dv.L * dv.d, d_Kcache, scores, nullptr, st)))
+    float *sp = score_partial_bytes(dv) ? reinterpret_cast<float *>(base + h.ws + kCounterBytes + partials_bytes(dv, Sv)) : nullptr;
+    if (int rc = cuda_rc(launch_score(dv, base + h.q, (int64_t)dv.H * dv.L * dv.d, (int64_t)dv.L * dv.d, d_Kcache, scores, nullptr, sp, st)))
         return rc;
-    if (int rc = cuda_rc(launch_topk(dv, scores, ids, st))) return rc;
+    if (int rc = cuda_rc(launch_topk(dv, scores, ids, st, sp, scores))) return rc;
     if (side && cudaStreamWaitEvent(st, ev_join, 0) != cudaSuccess) return PDLLM_ERR_CUDA;
     if (int rc = attn_impl(dv, base + h.q, d_Kcache, d_Vcache, ids, d_token_keep_idx, base + h.kd, base + h.vd, Sv,
                            base + h.o, reinterpret_cast<float *>(base + h.lse), nullptr, base + h.ws, true, nullptr, nullptr,

@@ -25,7 +25,9 @@ constexpr int kTileM = 128;   // query rows per CTA tile (UMMA M)
 constexpr int kTileN = 128;   // virtual KV rows per tile
 
 // ---- a2
-cudaError_t launch_topk(const Dims &s, const float *scores, int32_t *chunk_ids, cudaStream_t st);
+// partials / scores_out (optional, together): sum the chunk-score kernel's per-M-tile partials first (launch_score)
+cudaError_t launch_topk(const Dims &s, const float *scores, int32_t *chunk_ids, cudaStream_t st,
+                        const float *partials = nullptr, float *scores_out = nullptr);
 // ---- a3
 cudaError_t launch_gather_idx(const Dims &s, const int32_t *chunk_ids, const int32_t *keep, int32_t *gather_idx,
                               cudaStream_t st);
@@ -37,7 +39,7 @@ cudaError_t launch_combine(const float *O_part, const float *lse_part, int S, in
 // ---- a1: scores[b,g,n]
 // row_lse (optional): [B*H_kv, N, G*L_q] fp32, every scoring row's log-mass per chunk
 cudaError_t launch_score(const Dims &s, const void *Q, int64_t q_batch_stride, int64_t q_head_stride, const void *Kcache,
-                         float *scores, float *row_lse, cudaStream_t st);
+                         float *scores, float *row_lse, float *partials, cudaStream_t st);
 // ---- NEXT-1 (token_score.cu): e [B,H_kv,N,Cp] from row_lse; e_part: [m_tiles, B,H_kv,N,Cp] scratch when G*L_q > 128
 cudaError_t launch_token_scores(const Dims &s, const void *Q, int64_t q_batch_stride, int64_t q_head_stride,
                                 const void *Kcache, const float *row_lse, float *e, float *e_part, cudaStream_t st);

@@ -32,8 +32,10 @@ struct ScoreParams {
     int H_kv, G, N, Cp, L_q, rows;        // rows = G * L_q
     int m_tiles;
     int64_t units;                        // (b, g, M tile, chunk) work units, split evenly over the persistent CTAs
+    int64_t part_stride;                  // B*H_kv*N
     float c2, inv_rows;
-    int use_atomic, evict_first;
+    int use_atomic, evict_first;          // use_atomic: several M tiles add into scores[] (order not fixed)
+    float *partials;                      // or, when given: [m_tiles, B*H_kv*N] plain stores, summed in M-tile order by the consumer
 };
 
 template <int D>
@@ -317,7 +319,8 @@ score_kernel(const ScoreParams p, const __grid_constant__ CUtensorMap tmap128, c
     if (tid < n1 - n0) {
         const float tot = ((s_acc[tid * 4 + 0] + s_acc[tid * 4 + 1]) + (s_acc[tid * 4 + 2] + s_acc[tid * 4 + 3])) * p.inv_rows;
         float *dst = p.scores + (int64_t)bg * p.N + n0 + tid;
-        if (p.use_atomic) atomicAdd(dst, tot);
+        if (p.partials) p.partials[(int64_t)mt * p.part_stride + (int64_t)bg * p.N + n0 + tid] = tot;
+        else if (p.use_atomic) atomicAdd(dst, tot);
         else *dst = tot;
     }
     u += n1 - n0;
@@ -386,7 +389,7 @@ cudaError_t launch_score_d(const ScoreParams &p, const CUtensorMap &t128, const 
 }  // namespace
 
 cudaError_t launch_score(const Dims &s, const void *Q, int64_t q_batch_stride, int64_t q_head_stride, const void *Kcache,
-                         float *scores, float *row_lse, cudaStream_t st) {
+                         float *scores, float *row_lse, float *partials, cudaStream_t st) {
     ScoreParams p;
     p.Q = static_cast<const uint16_t *>(Q);
     p.q_batch_stride = q_batch_stride;
@@ -400,7 +403,9 @@ cudaError_t launch_score(const Dims &s, const void *Q, int64_t q_batch_stride, i
     p.units = (int64_t)BG * s.N * p.m_tiles;
     p.c2 = s.scale * 1.4426950408889634f;
     p.inv_rows = 1.0f / (float)p.rows;
-    p.use_atomic = p.m_tiles > 1;
+    p.partials = p.m_tiles > 1 ? partials : nullptr;
+    p.part_stride = (int64_t)BG * s.N;
+    p.use_atomic = p.m_tiles > 1 && !p.partials;
     p.evict_first = p.m_tiles == 1;
 
     CUtensorMap t128, t16;

@@ -14,8 +14,11 @@ __device__ __forceinline__ bool better(float v, int i, float bv, int bi) { retur
 // One warp per (b,g) row.  The row is staged in shared memory with 128-bit loads; K rounds of
 // "best remaining" (lane-local scan + shuffle arg-max) mark a bitmask; the mask is then emitted
 // in ascending index order (R6).  NaN is read as -inf.
+// `partials` (optional): [m_tiles, rows*N] per-M-tile score contributions of the chunk-score kernel; the row is then
+// their sum in M-tile order (bit-reproducible, unlike float atomics) and is also written to scores_out.
 __global__ void __launch_bounds__(kTopkWarps * 32) topk_kernel(const float *__restrict__ scores, int32_t *__restrict__ ids,
-                                                               int rows, int N, int K) {
+                                                               int rows, int N, int K, const float *__restrict__ partials,
+                                                               int m_tiles, float *__restrict__ scores_out) {
     extern __shared__ float smem_f[];
     // this kernel may have been launched under the kernel that writes the scores (programmatic dependent launch):
     // wait for that grid's completion and flush before the scores are read
@@ -29,7 +32,14 @@ __global__ void __launch_bounds__(kTopkWarps * 32) topk_kernel(const float *__re
     uint32_t *taken = reinterpret_cast<uint32_t *>(v + Npad);
     const float *src = scores + (size_t)row * N;
 
-    if ((N & 3) == 0 && ((reinterpret_cast<uintptr_t>(src) & 15) == 0)) {
+    if (partials) {
+        for (int i = lane; i < N; i += 32) {
+            float x = 0.f;
+            for (int mt = 0; mt < m_tiles; ++mt) x += partials[((size_t)mt * rows + row) * N + i];
+            scores_out[(size_t)row * N + i] = x;
+            v[i] = x == x ? x : -INFINITY;
+        }
+    } else if ((N & 3) == 0 && ((reinterpret_cast<uintptr_t>(src) & 15) == 0)) {
         for (int i = lane * 4; i < N; i += 128) {
             float4 x = *reinterpret_cast<const float4 *>(src + i);
             v[i] = x.x == x.x ? x.x : -INFINITY;
@@ -127,7 +137,8 @@ cudaError_t launch_validate(const Dims &s, const int32_t *chunk_ids, const int32
     return cudaGetLastError();
 }
 
-cudaError_t launch_topk(const Dims &s, const float *scores, int32_t *chunk_ids, cudaStream_t st) {
+cudaError_t launch_topk(const Dims &s, const float *scores, int32_t *chunk_ids, cudaStream_t st, const float *partials,
+                        float *scores_out) {
     const int rows = s.B * s.H_kv;
     const int Npad = (s.N + 3) & ~3, words = (s.N + 31) >> 5;
     const size_t smem = (size_t)kTopkWarps * (Npad + words) * sizeof(float);
@@ -148,7 +159,8 @@ cudaError_t launch_topk(const Dims &s, const float *scores, int32_t *chunk_ids, 
     cfg.attrs = attr;
     cfg.numAttrs = 1;
     const int N = s.N, K = s.K;
-    return cudaLaunchKernelEx(&cfg, topk_kernel, scores, chunk_ids, rows, N, K);
+    const int m_tiles = (s.G * s.L_q + kTileM - 1) / kTileM;
+    return cudaLaunchKernelEx(&cfg, topk_kernel, scores, chunk_ids, rows, N, K, partials, m_tiles, scores_out);
 }
 
 cudaError_t launch_gather_idx(const Dims &s, const int32_t *chunk_ids, const int32_t *keep, int32_t *gather_idx,

@@ -453,3 +453,24 @@ def test_scores_long_cta_runs(B, kw):
     ref = oracle.scores(inp["Q_dec"], inp["Kcache"], w.L_q)
     check_close(got, ref, SCORE_ABS, what="scores (long CTA runs)")
     check_exact(B.select_topk(shape, got), oracle.topk(ref, w.K))
+
+
+def test_step_gqa_scores_are_bit_reproducible(B):
+    """G*L_q > 128: the chunk-score kernel splits the scoring rows into several M tiles.  In pdllm_step their partial
+    scores go through the workspace and are summed in M-tile order by the top-K kernel (no float atomics), so repeated
+    steps give bit-identical scores; and they match the oracle."""
+    w, inp = _inputs("tiny", B=2, H=14, H_kv=2, d=128, N=24, C=200, K=3, keep=0.5, L_q=100, L_d=28)       # G = 7: 700 rows = 6 M tiles
+    dev = to_device(inp)
+    shape = B.Shape.of(w)
+    ref = oracle.step(inp["Q_dec"], inp["Kcache"], inp["Vcache"], inp["keep"], inp["K_dec"], inp["V_dec"], w.K, w.L_q)
+    ws = B.alloc_workspace(shape, 2)
+    first = B.step(shape, dev["Q_dec"], dev["Kcache"], dev["Vcache"], dev["keep"], dev["K_dec"], dev["V_dec"], n_splits=2, workspace=ws)
+    torch.cuda.synchronize()
+    check_close(first["scores"], ref["scores"], SCORE_ABS, what="scores")
+    check_exact(first["chunk_ids"], ref["ids"])
+    check_O(first["O"], ref["O"]); check_close(first["LSE"], ref["LSE"], LSE_ABS)
+    s0 = first["scores"].clone()
+    for _ in range(50):
+        out = B.step(shape, dev["Q_dec"], dev["Kcache"], dev["Vcache"], dev["keep"], dev["K_dec"], dev["V_dec"], n_splits=2, workspace=ws)
+        assert torch.equal(out["scores"].view(torch.int32), s0.view(torch.int32)), "scores changed between identical steps"
+    torch.cuda.synchronize()
