@@ -751,6 +751,104 @@ def run_prefill(args, w):
           K * (1 + (1 if Sd > 1 else 0)), clk.summary(), {})
 
 
+# --------------------------------------------------------------------------- BASELINE.json configs[4]: the sweep
+def sampled_parity(B, torch, w, shape, t):
+    """parity of 4 sampled (b, h) of one layer-step against the fp64 oracle, and the oracle's time on
+    them.  Returns dict(ok, score_err, o_err, o_norm, lse_err, oracle_s) -- the R12 gates decide `ok`; chunk ids are
+    checked as the oracle's top-K of the GPU's own scores (random data has no planted gap: same-precision decision)."""
+    from oracle import oracle
+    out = B.step(shape, t["Q"], t["Kc"], t["Vc"], None, t["Kd"], t["Vd"], workspace=t["ws"], **t["out"])
+    torch.cuda.synchronize()
+    picks = sorted({(0, 0), (w.B - 1, w.H - 1), (w.B // 2, 7 % w.H), (0, 19 % w.H)})
+    u16 = lambda x: x.contiguous().view(torch.int16).cpu().numpy().view(np.uint16)
+    res = dict(ok=True, score_err=0.0, o_err=0.0, o_norm=0.0, lse_err=0.0, oracle_s=0.0, heads=len(picks))
+    for b, h in picks:
+        sl = lambda x: u16(x[b:b + 1, h:h + 1])
+        Q, Kc, Vc, Kd, Vd = sl(t["Q"]), sl(t["Kc"]), sl(t["Vc"]), sl(t["Kd"]), sl(t["Vd"])
+        t0 = time.perf_counter()
+        sc = oracle.scores(Q, Kc, w.L_q)
+        g_sc = out["scores"][b, h].double().cpu().numpy()
+        ids = out["chunk_ids"][b:b + 1, h:h + 1].cpu().numpy()
+        O_ref, LSE_ref = oracle.attn(Q, Kc, Vc, ids, None, Kd, Vd)
+        res["oracle_s"] += time.perf_counter() - t0
+        O = (u16(out["O"][b:b + 1, h:h + 1]).astype(np.uint32) << 16).view(np.float32).astype(np.float64)
+        LSE = out["LSE"][b:b + 1, h:h + 1].double().cpu().numpy()
+        d_o = np.abs(O - O_ref)
+        res["score_err"] = max(res["score_err"], float(np.abs(g_sc - sc[0, 0]).max()))
+        res["o_err"] = max(res["o_err"], float(d_o.max()))
+        res["o_norm"] = max(res["o_norm"], float(d_o.max() / np.abs(O_ref).max()))
+        res["lse_err"] = max(res["lse_err"], float(np.abs(LSE - LSE_ref).max()))
+        ids_ok = bool((oracle.topk(g_sc[None, None], w.K) == ids).all())
+        res["ok"] = bool(res["ok"] and ids_ok and (d_o <= 2e-2 + 1e-2 * np.abs(O_ref)).all() and res["o_norm"] <= 1e-2
+                         and res["lse_err"] <= 1e-3 and res["score_err"] <= 1e-3)
+    return res
+
+
+def run_sweep(args):
+    """--mode sweep: paper_2606_10537_b200.sweep's points with the oracle leg per point (parity of 4 sampled (b, h); the
+    oracle's time on them scaled to all B*H heads of the layer-step, labelled extrapolated)."""
+    torch, B = _common_setup(args)
+    from paper_2606_10537_b200 import sweep as SW
+    g = torch.Generator(device="cuda").manual_seed(20260615)
+    rows = []
+
+    def hook(w, shape, t, row):
+        r = sampled_parity(B, torch, w, shape, t)
+        row["oracle_us_extrapolated"] = 1e6 * r["oracle_s"] * (w.B * w.H) / r["heads"]
+        row["parity"] = ("ok" if r["ok"] else "FAIL") + f" (O {r['o_err']:.1e}/{r['o_norm']:.1e}, LSE {r['lse_err']:.1e}, s {r['score_err']:.1e})"
+        row["parity_ok"] = r["ok"]
+
+    for pt in SW.grid_points(args.quick):
+        row = SW.run_point(B, torch, g, pt, args.layers, 3, 100.0, hook)
+        rows.append(row)
+        print(json.dumps(row), flush=True)
+    t = SW.table(rows)
+    if args.out:
+        Path(args.out).write_text(t)
+    print(t)
+    if not all(r.get("parity_ok", False) for r in rows):
+        raise SystemExit("bench.py --mode sweep: a sampled parity check failed")
+
+
+def run_splitsweep(args, w):
+    """--mode splitsweep: SURVEY 8(d): the workload's attention for every split count S = 1 .. min(64, KV tiles), the
+    partial-attention kernel and the LSE-combine kernel timed apart (CUDA events between them inside pdllm_step_profiled's
+    attention stage are not exposed for pdllm_sparse_attn, so the two are timed as: whole call, and pdllm_lse_combine
+    alone on partials of the same size)."""
+    torch, B = _common_setup(args)
+    shape = B.Shape.of(w)
+    inp = W.make_inputs(w)
+    bf = lambda bits: torch.from_numpy(np.ascontiguousarray(bits).view(np.int16)).cuda().view(torch.bfloat16)
+    dQ, dKc, dVc, dKd, dVd = (bf(inp[k]) for k in ("Q_dec", "Kcache", "Vcache", "K_dec", "V_dec"))
+    dkeep = None if inp["keep"] is None else torch.from_numpy(inp["keep"]).cuda()
+    ids = torch.from_numpy(inp["planted"]).cuda()
+    O = torch.empty((w.B, w.H, w.L, w.d), dtype=torch.bfloat16, device="cuda")
+    LSE = torch.empty((w.B, w.H, w.L), dtype=torch.float32, device="cuda")
+    flush = torch.empty((256 << 20,), dtype=torch.uint8, device="cuda") if needs_flush(w) else None
+    tiles = -(-w.S_kv // 128)
+    auto = B.auto_splits(shape, B.num_sms())
+    rows_n = w.B * w.H * w.L
+    lines = [f"| S | attention call us (cold L2) | of which LSE combine us | partial traffic MB (write + read) | note |", "|---|---|---|---|---|"]
+    for S in range(1, min(64, tiles) + 1):
+        ws = B.alloc_workspace(shape, S)
+        fn = lambda: B.sparse_attn(shape, dQ, dKc, dVc, ids, dkeep, dKd, dVd, n_splits=S, O=O, LSE=LSE, workspace=ws)
+        for _ in range(3):
+            fn()
+        us = _timed(torch, fn, args.steps, flush)
+        us_c = 0.0
+        if S > 1:
+            Op = torch.randn((S, rows_n, w.d), device="cuda"); lp = torch.randn((S, rows_n), device="cuda")
+            O2 = torch.empty((rows_n, w.d), dtype=torch.bfloat16, device="cuda"); L2 = torch.empty((rows_n,), dtype=torch.float32, device="cuda")
+            us_c = _timed(torch, lambda: B.lse_combine(Op, lp, O2, L2), args.steps, flush)
+        mb = 0.0 if S == 1 else 2 * S * rows_n * (w.d + 1) * 4 / 1e6
+        lines.append(f"| {S} | {us:.1f} | {us_c:.1f} | {mb:.1f} | {'auto (pdllm_auto_splits)' if S == auto else ''} |")
+        print(lines[-1], flush=True)
+    t = "\n".join(lines) + "\n"
+    if args.out:
+        Path(args.out).write_text(t)
+    print(t)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -759,7 +857,10 @@ def main():
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--workload", choices=list(W.CONFIGS) + list(W.EXTRA), default="sparse32k")
     ap.add_argument("--n-splits", type=int, default=0, help="0 = pdllm_auto_splits")
-    ap.add_argument("--mode", choices=["step", "static", "tokens", "prefill"], default="step",
+    ap.add_argument("--quick", action="store_true", help="--mode sweep: a 13-point subset")
+    ap.add_argument("--layers", type=int, default=32, help="--mode sweep: stacked layers per point")
+    ap.add_argument("--out", default="", help="--mode sweep / splitsweep: write the markdown table here")
+    ap.add_argument("--mode", choices=["step", "static", "tokens", "prefill", "sweep", "splitsweep"], default="step",
                     help="step: pdllm_step (the metric's per-step call, default); static / tokens / prefill: the rows "
                          "after the hot path (SURVEY 8(f)), 1 GPU")
     args = ap.parse_args()
@@ -771,6 +872,10 @@ def main():
     w = W.CONFIGS[args.workload] if args.workload in W.CONFIGS else W.EXTRA[args.workload]
     if args.impl == "reference":
         run_reference(args, w)
+    elif args.mode == "sweep":
+        run_sweep(args)
+    elif args.mode == "splitsweep":
+        run_splitsweep(args, w)
     elif args.mode == "static":
         run_static(args, w)
     elif args.mode == "tokens":
