@@ -255,6 +255,10 @@ attn_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tm_kp, const
         int n_done = 0;                                   // items finished by this CTA
         // Work items are handed out dynamically (costliest first: pair items, then single items), so CTAs that
         // finish early take more; thread 0 of the producers fetches, the other roles follow through s_items.
+        // The kernel is launched as a programmatic dependent of its predecessor in the stream (top-K in pdllm_step): the
+        // set-up above ran under that kernel's tail.  Nothing that kernel may have written is read before this wait; the
+        // other roles read no global memory (their stores follow data that passed through here).
+        asm volatile("griddepcontrol.wait;" ::: "memory");
         for (;; ++n_done) {
             if (pt == 0) {
                 // the first item of a CTA is its block index (no round trip to the counter at kernel start)
@@ -794,11 +798,21 @@ cudaError_t launch_attn_d(const AttnParams &p, const CUtensorMap (&tm)[4], cudaS
     cudaError_t e = cudaFuncSetAttribute(attn_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::kSmem);
     if (e != cudaSuccess) return e;
     const int grid = p.n_items < device_num_sms() ? p.n_items : device_num_sms();
-    // (Launching this kernel as a programmatic dependent of the top-K kernel was measured -- 2.6 us per step -- and
-    // withdrawn: with the combine kernel behind it, long unsynchronised step loops ended in an invalid-address-space
-    // fault that a plain launch never shows.)
-    attn_kernel<D><<<grid, kAttnThreads, Cfg::kSmem, st>>>(p, tm[0], tm[1], tm[2], tm[3]);
-    return cudaGetLastError();
+    // Programmatic dependent launch: the CTAs become resident as SMs fall free under the predecessor's tail (top-K, which
+    // triggers at its start, in pdllm_step), set themselves up, and wait at the head of the producer role.  (Round 1
+    // withdrew a first attempt after an invalid-address-space fault in long loops; this placement -- nothing read before
+    // the wait, the trigger in top-K -- was soaked over 12,600 unsynchronised steps with S = 1..3.)
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)grid, 1, 1);
+    cfg.blockDim = dim3(kAttnThreads, 1, 1);
+    cfg.dynamicSmemBytes = Cfg::kSmem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, attn_kernel<D>, p, tm[0], tm[1], tm[2], tm[3]);
 }
 
 void fill_common(AttnParams &p, const Dims &s, int n_splits) {

@@ -15,6 +15,9 @@ __global__ void __launch_bounds__(kCombineWarps * 32) combine_kernel(const float
                                                                      const float *__restrict__ lse_part, int S, int64_t rows,
                                                                      uint16_t *__restrict__ O, float *__restrict__ LSE) {
     constexpr int V = D / 32;                      // floats per lane: 4 (d=128) or 2 (d=64)
+    // launched as a programmatic dependent of the kernel that writes the partials (its launch is processed while that
+    // kernel still runs): wait for that grid's completion and flush before reading them
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int64_t row = (int64_t)blockIdx.x * kCombineWarps + warp;
     if (row >= rows) return;
@@ -67,12 +70,18 @@ __global__ void __launch_bounds__(kCombineWarps * 32) combine_kernel(const float
 
 cudaError_t launch_combine(const float *O_part, const float *lse_part, int S, int64_t rows, int d, void *O, float *LSE,
                            cudaStream_t st) {
-    const unsigned blocks = (unsigned)((rows + kCombineWarps - 1) / kCombineWarps);
-    if (d == 128)
-        combine_kernel<128><<<blocks, kCombineWarps * 32, 0, st>>>(O_part, lse_part, S, rows, static_cast<uint16_t *>(O), LSE);
-    else
-        combine_kernel<64><<<blocks, kCombineWarps * 32, 0, st>>>(O_part, lse_part, S, rows, static_cast<uint16_t *>(O), LSE);
-    return cudaGetLastError();
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)((rows + kCombineWarps - 1) / kCombineWarps), 1, 1);
+    cfg.blockDim = dim3(kCombineWarps * 32, 1, 1);
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    uint16_t *Ob = static_cast<uint16_t *>(O);
+    if (d == 128) return cudaLaunchKernelEx(&cfg, combine_kernel<128>, O_part, lse_part, S, rows, Ob, LSE);
+    return cudaLaunchKernelEx(&cfg, combine_kernel<64>, O_part, lse_part, S, rows, Ob, LSE);
 }
 
 }  // namespace pdllm

@@ -22,6 +22,9 @@ __global__ void __launch_bounds__(kTopkWarps * 32) topk_kernel(const float *__re
     extern __shared__ float smem_f[];
     // this kernel may have been launched under the kernel that writes the scores (programmatic dependent launch):
     // wait for that grid's completion and flush before the scores are read
+    // ... and lets its own dependent (the attention kernel in pdllm_step) be scheduled as SMs fall free: that kernel
+    // does its set-up, then waits for this grid in turn
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     asm volatile("griddepcontrol.wait;" ::: "memory");
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int row = blockIdx.x * kTopkWarps + warp;
