@@ -43,10 +43,10 @@ SPEC_PEAKS = {"hbm_gbs": 8000.0, "bf16_tflops": 2250.0}      # the peaks BASELIN
 # dram__bytes_read.sum + dram__bytes_write.sum per launch, copied from the committed `ncu --set full` capture named in
 # NCU_TRAFFIC_SOURCE (NOT measured by the run that prints it: ncu cannot run inside a timed bench); keyed by
 # (workload, kernel); None where no capture exists for that pair.
-NCU_TRAFFIC_SOURCE = "profiles/r1_ncu_full_v6.md (ncu capture of these kernels on another box; not measured in this run)"
+NCU_TRAFFIC_SOURCE = "profiles/r2_ncu_full.md (ncu --set full capture of these kernels; not measured in this run)"
 NCU_TRAFFIC_BYTES = {
-    ("sparse32k", "score_kernel"): 1081.260e6 + 3.529472e6,
-    ("sparse32k", "attn_kernel"): 149.460e6 + 5.651712e6,
+    ("sparse32k", "score_kernel"): 1081.249e6 + 3.572480e6,
+    ("sparse32k", "attn_kernel"): 148.781e6 + 6.031872e6,
 }
 
 
