@@ -774,11 +774,14 @@ attn_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tm_kp, const
                                     reinterpret_cast<uint4 *>(dst)[q4] = make_uint4(u[4 * q4], u[4 * q4 + 1], u[4 * q4 + 2], u[4 * q4 + 3]);
                             }
                         } else {
-                            float4 *dst =
-                                reinterpret_cast<float4 *>(p.O_part + ((int64_t)it.split * p.total_rows + grow) * D + ch * 32);
+                            // whole 32-byte sectors per lane and store (rows are 4*D bytes apart; the workspace is 256-byte
+                            // aligned): 16-byte stores would each write half a sector
+                            float *dst = p.O_part + ((int64_t)it.split * p.total_rows + grow) * D + ch * 32;
 #pragma unroll
-                            for (int q4 = 0; q4 < 8; ++q4)
-                                dst[q4] = make_float4(f[q4 * 4 + 0], f[q4 * 4 + 1], f[q4 * 4 + 2], f[q4 * 4 + 3]);
+                            for (int q8 = 0; q8 < 4; ++q8)
+                                st_global_v8(dst + q8 * 8, __float_as_uint(f[q8 * 8 + 0]), __float_as_uint(f[q8 * 8 + 1]),
+                                             __float_as_uint(f[q8 * 8 + 2]), __float_as_uint(f[q8 * 8 + 3]), __float_as_uint(f[q8 * 8 + 4]),
+                                             __float_as_uint(f[q8 * 8 + 5]), __float_as_uint(f[q8 * 8 + 6]), __float_as_uint(f[q8 * 8 + 7]));
                         }
                     }
                 }
