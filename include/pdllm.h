@@ -89,7 +89,7 @@ typedef struct {
 
 /* ---- host-only, pure helpers (no CUDA call, usable without a GPU) ---------- */
 
-int pdllm_version(void);                       /* e.g. 100 = 0.1.0 */
+int pdllm_version(void);                       /* 200 = 0.2.0 (round 2: pdllm_step_host takes the side stream) */
 const char *pdllm_strerror(int status);        /* static string, never NULL */
 
 /* a6 (S8(a); P:189-191 fixes S = 4, NS: "chosen from N*K*C and the number of
@@ -103,9 +103,12 @@ const char *pdllm_strerror(int status);        /* static string, never NULL */
 int32_t pdllm_auto_splits(const pdllm_shape *shape, int32_t num_sms);
 
 /* Bytes of scratch pdllm_sparse_attn / pdllm_step need for n_splits splits
- * (n_splits == 0: the auto choice for num_sms): always >= 256 (the persistent
- * attention kernel's work-item counter, cleared by the call itself), plus the fp32
- * partials when there is more than one split.  Returns 0 for an invalid shape. */
+ * (n_splits == 0: the auto choice for num_sms; num_sms <= 0: the current device's
+ * SM count.  Should the auto choice of the device that later runs the call differ,
+ * the call takes the largest split count this many bytes hold): always >= 256 (the
+ * persistent attention kernel's work-item counter, cleared by the call itself), plus
+ * the fp32 partials when there is more than one split, plus -- when G*L_q > 128 --
+ * the per-M-tile chunk-score partials of pdllm_step.  Returns 0 for an invalid shape. */
 size_t pdllm_workspace_bytes(const pdllm_shape *shape, int32_t n_splits, int32_t num_sms);
 
 /* Bytes of device scratch pdllm_step_host needs (staging of the per-step tensors
@@ -120,7 +123,11 @@ size_t pdllm_step_host_scratch_bytes(const pdllm_shape *shape, int32_t n_splits,
  *           (strides in elements, multiples of 8) -- lets the first L_q rows of
  *           Q_dec [B,H,L,d] be scored in place
  *   Kcache  device bf16 [B,H_kv,N,C+1,d]
- *   scores  device fp32 [B,H_kv,N] (out)                                          */
+ *   scores  device fp32 [B,H_kv,N] (out)
+ * Reproducibility: bit-identical from run to run when G*L_q <= 128.  Above that the
+ * scoring rows span several 128-row M tiles whose contributions this standalone call
+ * adds with float atomics (last bits may vary); pdllm_step and pdllm_score_tokens sum
+ * them in a fixed order through their scratch and are bit-reproducible.            */
 int pdllm_score_chunks(const pdllm_shape *shape, const void *Q, int64_t q_batch_stride,
                        int64_t q_head_stride, const void *Kcache, float *scores,
                        pdllm_stream_t stream);

@@ -163,7 +163,7 @@ using namespace pdllm;
 
 extern "C" {
 
-int pdllm_version(void) { return 100; }
+int pdllm_version(void) { return 200; }
 
 const char *pdllm_strerror(int status) {
     switch (status) {
