@@ -474,3 +474,18 @@ def test_step_gqa_scores_are_bit_reproducible(B):
         out = B.step(shape, dev["Q_dec"], dev["Kcache"], dev["Vcache"], dev["keep"], dev["K_dec"], dev["V_dec"], n_splits=2, workspace=ws)
         assert torch.equal(out["scores"].view(torch.int32), s0.view(torch.int32)), "scores changed between identical steps"
     torch.cuda.synchronize()
+
+
+@pytest.mark.parametrize("where", [150, 300, 640])
+@pytest.mark.parametrize("L_q,L_d", [(64, 64), (100, 284)])
+def test_attn_logit_jump_beyond_the_soft_range(B, where, L_q, L_d):
+    """One cached key whose logit sits ~85 nats (> 100 octaves) above everything the row has seen when its tile comes up:
+    the single-pass softmax would form P = 2^120; the row sum trips the hard limit and the tile is redone behind an exact
+    row max (the careful pass), with l and O rescaled.  Pair and single items, the key in the 2nd / 3rd / 6th KV tile."""
+    w, inp = _inputs("tiny", C=400, N=3, K=3, keep=1.0, L_q=L_q, L_d=L_d, H=2, H_kv=2, d=128)       # K = N: virtual row = cache row
+    u = np.zeros(w.d, np.float32); u[::2] = 1.0; u /= np.linalg.norm(u)
+    Q = W.bf16_bits_to_f32(inp["Q_dec"]) + 4.0 * u
+    Kc = W.bf16_bits_to_f32(inp["Kcache"]).copy().reshape(w.B, w.H_kv, w.N * w.Cp, w.d)
+    Kc[:, :, where] += 240.0 * u                                  # logit ~ (1/sqrt(128)) * 4 * 240 = 85 nats
+    inp["Q_dec"], inp["Kcache"] = W.f32_to_bf16_bits(Q), W.f32_to_bf16_bits(Kc.reshape(w.B, w.H_kv, w.N, w.Cp, w.d))
+    _attn_case(B, w, inp, [1, 2])
