@@ -39,6 +39,15 @@ def test_paper_shape_facts_match_the_cache_layout():
     assert bos_rows == [int(i) * w.Cp for i in ids[0, 0]]                           # one BOS row per selected chunk
     # the paper's decode-kernel shape is expressible: GQA 32/8, L_d = 32, S = 4
     assert f["fig5b_query_heads"] % f["fig5b_kv_heads"] == 0 and f["fig5b_splits"] == 4 and f["fig5b_decode_tokens"] == 32
+    # NEXT-4 workloads (R25): the Fig. 5(b) shape with the paper's query window, strict R8 rows
+    for name in ("fig5b_8k", "fig5b_16k", "fig5b_32k"):
+        x = W.EXTRA[name]
+        assert (x.H, x.H_kv, x.L_d, x.L_q) == (f["fig5b_query_heads"], f["fig5b_kv_heads"], f["fig5b_decode_tokens"], f["query_window_tokens"])
+        assert x.strict and x.L == x.L_d and x.L_s == x.L_q + x.L_d and x.G * x.L == 128 and x.C == f["chunk_tokens"]
+    # top-B = 512 of C = 1024 is config C3's 50 % keep: Bk = 1 + B
+    c3 = W.CONFIGS["dream16k"]
+    assert c3.C == f["chunk_tokens"] and c3.Bk == 1 + f["top_b_tokens"]
+    assert f["timing_pseudo_label_tokens"] == 16 and f["timing_generated_tokens"] == f["fig5b_decode_tokens"]
 
 
 def test_oracle_reproduces_its_stored_results_on_tiny():
