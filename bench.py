@@ -457,7 +457,7 @@ def run_ours(args, w):
             "e2e": {"value": e2e_us, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "call": "pdllm_step_host (pinned host Q_dec/K_dec/V_dec in; O, LSE, chunk ids out; KV cache resident)",
                     "result_ok": e2e_ok},
-            "gpu_launches": K * (3 + (1 if S > 1 else 0)),
+            "gpu_launches": K * ((2 if w.N <= B.FOLD_MAX_N else 3) + (1 if S > 1 else 0)),   # a2 runs inside a4 up to FOLD_MAX_N chunks
             "cpu_baseline": cpu, "clocks": clocks, "planted_chunks_recovered": ok}
     print(json.dumps(line))
     if world > 1:

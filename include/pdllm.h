@@ -178,7 +178,13 @@ int pdllm_lse_combine(const float *O_part, const float *lse_part, int32_t S, int
 /* ---- the per-step call: a1 -> a2 -> (a3) -> a4 -> a5 as one enqueue sequence ---
  * Rows 0..L_q-1 of every head of Q_dec are the scoring rows (R8).
  * scores_out [B,H_kv,N] fp32 and chunk_ids_out [B,H_kv,K] int32 are required
- * device outputs (they carry the data between the kernels).                       */
+ * device outputs (they carry the data between the kernels).
+ * With N <= PDLLM_FOLD_MAX_N chunks and gather_idx_out == NULL, a2 runs inside the
+ * a4 kernel (each work item ranks its group's scores; same order, same ties, same
+ * ids and scores written as pdllm_select_topk) and the sequence is one launch
+ * shorter; otherwise a2 is a kernel of its own.  PDLLM_NO_FOLD=1 in the environment
+ * (read once) keeps it apart always.                                              */
+#define PDLLM_FOLD_MAX_N 128
 int pdllm_step(const pdllm_shape *shape, const void *Q_dec, const void *Kcache, const void *Vcache,
                const int32_t *token_keep_idx, const void *K_dec, const void *V_dec, int32_t n_splits,
                float *scores_out, int32_t *chunk_ids_out, void *O, float *LSE,
@@ -190,7 +196,8 @@ int pdllm_step(const pdllm_shape *shape, const void *Q_dec, const void *Kcache, 
  * (cudaEvent_t handles created by the caller with timing enabled, passed as opaque
  * pointers; a NULL member is skipped) on `stream` at the stage boundaries, so that
  * a harness can attribute the step's device time to a1 / a2 / a3-a5 inside the same
- * timed region.  ev == NULL is exactly pdllm_step. */
+ * timed region.  ev == NULL is exactly pdllm_step; with events a2 is always a
+ * kernel of its own (there is a boundary to stamp). */
 typedef struct {
     void *begin;         /* before a1 */
     void *after_score;   /* after a1 (chunk-score reduction) */

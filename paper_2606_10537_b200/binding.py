@@ -16,6 +16,7 @@ from pathlib import Path
 _PKG = Path(__file__).resolve().parent
 _LIB_PATH = _PKG / "libpdllm.so"
 _lib = None
+FOLD_MAX_N = 128            # include/pdllm.h PDLLM_FOLD_MAX_N: up to this many chunks pdllm_step runs a2 inside the a4 kernel
 
 EXPORTS = [
     "pdllm_version", "pdllm_strerror", "pdllm_auto_splits", "pdllm_workspace_bytes",

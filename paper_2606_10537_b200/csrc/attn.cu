@@ -39,6 +39,7 @@ constexpr int kAttnThreads = 2 * kSoftmaxThreads + kProducerThreads + 128;     /
 // register budgets after the roles part ways (setmaxnreg; 256 * 176 + 128 * 104 + 128 * 56 = 65536)
 constexpr int kSoftmaxRegs = 176, kProducerRegs = 104, kOtherRegs = 56;
 constexpr int kInvalidRow = INT32_MIN;
+constexpr int kFoldMaxN = PDLLM_FOLD_MAX_N;              // top-K is folded into the kernel up to this many chunks
 constexpr float kRescaleThreshold = 8.0f;                 // log2 units: P stays <= 2^8 between reference-max updates
 
 struct AttnParams {
@@ -54,6 +55,12 @@ struct AttnParams {
     int32_t *work_counter;                                // zeroed before launch: next work item to hand out
     int64_t total_rows;                                   // B*H*L
     float c2;                                             // scale * log2(e)
+    // a2 folded into the kernel (pdllm_step, N <= kFoldMaxN): the group's chunk ids are chosen here from the scores
+    const float *fold_scores;                             // [B*H_kv, N] or, with fold_m_tiles > 1, [m_tiles, B*H_kv, N] partials
+    int fold_m_tiles;
+    int64_t fold_stride;                                  // B*H_kv*N
+    int32_t *fold_ids_out;                                // [B*H_kv, K]
+    float *fold_scores_out;                               // [B*H_kv, N], written when the scores come as partials
 };
 
 struct Item {
@@ -160,6 +167,7 @@ attn_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tm_kp, const
     __shared__ uint64_t bars[BAR_KV + 2 * (ST + 1)];
     __shared__ uint32_t tmem_slot;
     __shared__ int32_t s_items[4];                        // the CTA's next work items (ring, published by the producers)
+    __shared__ int32_t s_ids[64];                         // folded top-K: the current item's chunk ids
     __shared__ float s_ml[kSoftmaxThreads][3];            // single items: stream 1's (m_ref, l, O scale) for the in-CTA merge
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -275,8 +283,59 @@ attn_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tm_kp, const
             const uint16_t *Kd = p.Kd + bg * p.L_s * D, *Vd = p.Vd + bg * p.L_s * D;
             const int32_t *keep = p.keep ? p.keep + bg * p.N * p.Bk : nullptr;
             // the group's K <= 64 chunk ids live in two registers per lane (lane l: ids[l], ids[l + 32])
-            const int ids_lo = (!p.contig && lane < p.K) ? __ldg(p.ids + bg * p.K + lane) : 0;
-            const int ids_hi = (!p.contig && lane + 32 < p.K) ? __ldg(p.ids + bg * p.K + lane + 32) : 0;
+            int ids_lo = 0, ids_hi = 0;
+            if (p.fold_scores) {
+                // a2 (R6) inside the kernel: producer warp 0 ranks the group's N <= 128 scores -- rank = number of
+                // chunks ahead in the (score descending, index ascending) order; the K chunks of rank < K are the selection
+                // -- and lists them in ascending index order.  Every item of the group arrives at the same list.
+                if (pw == 0) {
+                    float v[kFoldMaxN / 32];
+                    int rank[kFoldMaxN / 32];
+#pragma unroll
+                    for (int r = 0; r < kFoldMaxN / 32; ++r) {
+                        const int idx = r * 32 + lane;
+                        float x = -INFINITY;
+                        if (idx < p.N) {
+                            x = 0.f;
+                            for (int mt = 0; mt < p.fold_m_tiles; ++mt) x += p.fold_scores[mt * p.fold_stride + bg * p.N + idx];
+                            if (p.fold_scores_out && it.q0 == 0 && it.split == 0) p.fold_scores_out[bg * p.N + idx] = x;
+                            if (x != x) x = -INFINITY;        // NaN counts as -inf
+                        }
+                        v[r] = x;
+                        rank[r] = 0;
+                    }
+#pragma unroll
+                    for (int r2 = 0; r2 < kFoldMaxN / 32; ++r2) {
+                        if (r2 * 32 >= p.N) break;
+                        for (int l2 = 0; l2 < 32 && r2 * 32 + l2 < p.N; ++l2) {
+                            const float o = __shfl_sync(0xffffffffu, v[r2], l2);
+                            const int idx2 = r2 * 32 + l2;
+#pragma unroll
+                            for (int r = 0; r < kFoldMaxN / 32; ++r)
+                                if (r * 32 < p.N) rank[r] += (o > v[r] || (o == v[r] && idx2 < r * 32 + lane)) ? 1 : 0;
+                        }
+                    }
+                    int base = 0;
+#pragma unroll
+                    for (int r = 0; r < kFoldMaxN / 32; ++r) {
+                        const int idx = r * 32 + lane;
+                        const bool sel = idx < p.N && rank[r] < p.K;
+                        const uint32_t m = __ballot_sync(0xffffffffu, sel);
+                        if (sel) {
+                            const int pos = base + __popc(m & ((1u << lane) - 1u));
+                            s_ids[pos] = idx;
+                            if (it.q0 == 0 && it.split == 0) p.fold_ids_out[bg * p.K + pos] = idx;
+                        }
+                        base += __popc(m);
+                    }
+                }
+                asm volatile("bar.sync 1, 128;" ::: "memory");
+                ids_lo = lane < p.K ? s_ids[lane] : 0;
+                ids_hi = lane + 32 < p.K ? s_ids[lane + 32] : 0;
+            } else if (!p.contig) {
+                ids_lo = lane < p.K ? __ldg(p.ids + bg * p.K + lane) : 0;
+                ids_hi = lane + 32 < p.K ? __ldg(p.ids + bg * p.K + lane + 32) : 0;
+            }
             // a3: virtual row -> cache row (>= 0) / decode row (< 0) / invalid; one row per producer thread.  The index
             // is kept as (base, raw) with raw = the keep-list entry still in flight: the sum is only formed when the
             // row is issued, one load later, so the global load latency hides behind the previous tile's cp.async.
@@ -837,6 +896,8 @@ void fill_common(AttnParams &p, const Dims &s, int n_splits) {
 
 }  // namespace
 
+bool attn_can_fold_topk(const Dims &d) { return !d.contig && d.N <= kFoldMaxN; }
+
 int kv_tiles(const Dims &d) {
     if (!d.contig) return (d.S_kv + kTileN - 1) / kTileN;
     return (d.S_pre + kTileN - 1) / kTileN + (d.L_s + kTileN - 1) / kTileN;
@@ -844,7 +905,7 @@ int kv_tiles(const Dims &d) {
 
 cudaError_t launch_attn(const Dims &s, const void *Q_dec, const void *Kcache, const void *Vcache, const int32_t *chunk_ids,
                         const int32_t *keep, const void *K_dec, const void *V_dec, int n_splits, void *O, float *LSE,
-                        float *O_part, float *lse_part, int32_t *work_counter, cudaStream_t st) {
+                        float *O_part, float *lse_part, int32_t *work_counter, cudaStream_t st, const AttnFold *fold) {
     AttnParams p;
     p.Q = static_cast<const uint16_t *>(Q_dec);
     p.Kc = static_cast<const uint16_t *>(Kcache);
@@ -859,6 +920,17 @@ cudaError_t launch_attn(const Dims &s, const void *Q_dec, const void *Kcache, co
     p.lse_part = lse_part;
     p.work_counter = work_counter;
     fill_common(p, s, n_splits);
+    p.fold_scores = nullptr;
+    p.fold_m_tiles = 1;
+    p.fold_stride = (int64_t)s.B * s.H_kv * s.N;
+    p.fold_ids_out = nullptr;
+    p.fold_scores_out = nullptr;
+    if (fold) {
+        p.fold_scores = fold->partials ? fold->partials : fold->scores;
+        p.fold_m_tiles = fold->partials ? (s.G * s.L_q + kTileM - 1) / kTileM : 1;
+        p.fold_ids_out = fold->ids_out;
+        p.fold_scores_out = fold->partials ? fold->scores_out : nullptr;
+    }
     CUtensorMap tm[4];
     if (s.contig) {
         // contiguous mode: Kcache / Vcache are [B*H_kv, S_pre, d] (compact static cache, or a prefill sequence's K / V);

@@ -238,6 +238,12 @@ int pdllm_lse_combine(const float *O_part, const float *lse_part, int32_t S, int
 
 namespace {
 
+// PDLLM_NO_FOLD=1 keeps a2 a kernel of its own in pdllm_step (A/B switch; read once)
+bool no_fold() {
+    static const bool v = [] { const char *e = getenv("PDLLM_NO_FOLD"); return e && e[0] == '1'; }();
+    return v;
+}
+
 int record(void *ev, cudaStream_t st) {
     if (!ev) return PDLLM_OK;
     return cuda_rc(cudaEventRecord(static_cast<cudaEvent_t>(ev), st));
@@ -246,7 +252,8 @@ int record(void *ev, cudaStream_t st) {
 // a3 + a4 + a5 on validated arguments; ev_mid / ev_end (may be NULL) are recorded after a4 / a5.
 int attn_impl(const Dims &d, const void *Q_dec, const void *Kcache, const void *Vcache, const int32_t *chunk_ids,
               const int32_t *token_keep_idx, const void *K_dec, const void *V_dec, int S, void *O, float *LSE,
-              int32_t *gather_idx_out, void *workspace, bool counter_zeroed, void *ev_mid, void *ev_end, cudaStream_t st) {
+              int32_t *gather_idx_out, void *workspace, bool counter_zeroed, void *ev_mid, void *ev_end, cudaStream_t st,
+              const AttnFold *fold = nullptr) {
     int32_t *counter = static_cast<int32_t *>(workspace);
     if (!counter_zeroed)
         if (int rc = cuda_rc(cudaMemsetAsync(counter, 0, sizeof(int32_t), st))) return rc;
@@ -260,7 +267,7 @@ int attn_impl(const Dims &d, const void *Q_dec, const void *Kcache, const void *
                                              align_up((size_t)S * rows * d.d * sizeof(float), 256));
     }
     if (int rc = cuda_rc(launch_attn(d, Q_dec, Kcache, Vcache, chunk_ids, token_keep_idx, K_dec, V_dec, S, O, LSE, O_part,
-                                     lse_part, counter, st)))
+                                     lse_part, counter, st, fold)))
         return rc;
     if (int rc = record(ev_mid, st)) return rc;
     if (S > 1)
@@ -484,6 +491,14 @@ int pdllm_step_profiled(const pdllm_shape *shape, const void *Q_dec, const void 
                                        : nullptr;
     if (int rc = cuda_rc(launch_score(d, Q_dec, (int64_t)d.H * d.L * d.d, (int64_t)d.L * d.d, Kcache, scores_out, nullptr, sp, st)))
         return rc;
+    // a2 inside the attention kernel (one launch fewer; the attention becomes the score kernel's programmatic
+    // dependent) when the chunk count allows it, no gather-index export wants the ids ahead of a4 and no stage
+    // events are asked for; the ids and scores written are those the top-K kernel would write
+    if (!ev && !gather_idx_out && attn_can_fold_topk(d) && !no_fold()) {
+        AttnFold fold{scores_out, sp, chunk_ids_out, scores_out};
+        return attn_impl(d, Q_dec, Kcache, Vcache, chunk_ids_out, token_keep_idx, K_dec, V_dec, S, O, LSE, nullptr,
+                         workspace, true, nullptr, nullptr, st, &fold);
+    }
     if (int rc = record(ev ? ev->after_score : nullptr, st)) return rc;
     if (int rc = cuda_rc(launch_topk(d, scores_out, chunk_ids_out, st, sp, scores_out))) return rc;
     if (int rc = record(ev ? ev->after_topk : nullptr, st)) return rc;
@@ -544,11 +559,14 @@ int pdllm_step_host(const pdllm_shape *shape, const void *h_Q_dec, const void *h
     float *sp = score_partial_bytes(dv) ? reinterpret_cast<float *>(base + h.ws + kCounterBytes + partials_bytes(dv, Sv)) : nullptr;
     if (int rc = cuda_rc(launch_score(dv, base + h.q, (int64_t)dv.H * dv.L * dv.d, (int64_t)dv.L * dv.d, d_Kcache, scores, nullptr, sp, st)))
         return rc;
-    if (int rc = cuda_rc(launch_topk(dv, scores, ids, st, sp, scores))) return rc;
+    const bool fold_topk = attn_can_fold_topk(dv) && !no_fold();
+    if (!fold_topk)
+        if (int rc = cuda_rc(launch_topk(dv, scores, ids, st, sp, scores))) return rc;
     if (side && cudaStreamWaitEvent(st, ev_join, 0) != cudaSuccess) return PDLLM_ERR_CUDA;
+    AttnFold fold{scores, sp, ids, scores};
     if (int rc = attn_impl(dv, base + h.q, d_Kcache, d_Vcache, ids, d_token_keep_idx, base + h.kd, base + h.vd, Sv,
                            base + h.o, reinterpret_cast<float *>(base + h.lse), nullptr, base + h.ws, true, nullptr, nullptr,
-                           st))
+                           st, fold_topk ? &fold : nullptr))
         return rc;
     if (cudaMemcpyAsync(h_O, base + h.o, qb, cudaMemcpyDeviceToHost, st) != cudaSuccess) return PDLLM_ERR_CUDA;
     if (cudaMemcpyAsync(h_LSE, base + h.lse, (size_t)d.B * d.H * d.L * 4, cudaMemcpyDeviceToHost, st) != cudaSuccess)

@@ -47,9 +47,17 @@ cudaError_t launch_topb(const Dims &s, const float *token_scores, int32_t *keep,
 int topb_max_cp();
 // ---- a3+a4 into O / LSE (n_splits == 1) or into the partials (n_splits > 1: launch_combine follows);
 // work_counter: one zeroed int32 (the persistent kernel's work-item counter)
+// fold (optional): a2 inside the attention kernel -- the chunk ids are chosen from `scores` (or the per-M-tile
+// `partials`, summed in M-tile order and written to scores_out) and written to ids_out; chunk_ids is then unused
+struct AttnFold {
+    const float *scores, *partials;
+    int32_t *ids_out;
+    float *scores_out;
+};
+bool attn_can_fold_topk(const Dims &d);
 cudaError_t launch_attn(const Dims &s, const void *Q_dec, const void *Kcache, const void *Vcache, const int32_t *chunk_ids,
                         const int32_t *keep, const void *K_dec, const void *V_dec, int n_splits, void *O, float *LSE,
-                        float *O_part, float *lse_part, int32_t *work_counter, cudaStream_t st);
+                        float *O_part, float *lse_part, int32_t *work_counter, cudaStream_t st, const AttnFold *fold = nullptr);
 
 int device_num_sms();
 // KV tiles of 128 rows one query tile walks (gather mode: ceil(S_kv / 128); contiguous mode: prefix and decode rows

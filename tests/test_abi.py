@@ -27,6 +27,11 @@ def test_library_exports_every_declared_symbol():
     assert sorted(B.EXPORTS) == names
 
 
+def test_header_constants_match_the_binding():
+    hdr = (ROOT / "include" / "pdllm.h").read_text()
+    assert int(re.search(r"#define\s+PDLLM_FOLD_MAX_N\s+(\d+)", hdr).group(1)) == B.FOLD_MAX_N
+
+
 def test_version_and_strerror():
     lib = B.lib()
     assert lib.pdllm_version() >= 100

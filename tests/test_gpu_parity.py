@@ -489,3 +489,45 @@ def test_attn_logit_jump_beyond_the_soft_range(B, where, L_q, L_d):
     Kc[:, :, where] += 240.0 * u                                  # logit ~ (1/sqrt(128)) * 4 * 240 = 85 nats
     inp["Q_dec"], inp["Kcache"] = W.f32_to_bf16_bits(Q), W.f32_to_bf16_bits(Kc.reshape(w.B, w.H_kv, w.N, w.Cp, w.d))
     _attn_case(B, w, inp, [1, 2])
+
+
+@pytest.mark.parametrize("kw", [
+    dict(N=64, C=40, K=8, keep=0.5, d=128, H=4, H_kv=4, L_q=32, L_d=64),              # the C4 chunk count
+    dict(N=100, C=24, K=33, keep=1.0, d=64, H=4, H_kv=2, L_q=16, L_d=40),             # ragged 4th id register, K > 32
+    dict(N=128, C=16, K=5, keep=1.0, d=128, H=14, H_kv=2, L_q=40, L_d=8),             # the fold's bound; G*L_q = 280: score partials
+    dict(N=129, C=16, K=5, keep=1.0, d=128, H=2, H_kv=2, L_q=16, L_d=8),              # just beyond it: the top-K kernel runs
+    dict(N=1, C=300, K=1, keep=0.3, d=128, H=2, H_kv=1, L_q=8, L_d=24),               # one chunk
+])
+def test_step_topk_inside_attention_matches_topk_kernel(B, kw):
+    """pdllm_step chooses the chunks inside the attention kernel when N <= 128 (a2 folded into a4); with stage events
+    or a gather-index export the separate top-K kernel runs.  Both must give the oracle's ids and bit-identical
+    scores, ids, O and LSE -- also with exact score ties (duplicated chunks), which go to the lower index."""
+    w, inp = _inputs("tiny", **kw)
+    if w.N >= 8:                                                  # chunks 5 and 6 become copies of 2 and 1: exact ties
+        for name in ("Kcache", "Vcache"):
+            inp[name][:, :, 5] = inp[name][:, :, 2]
+            inp[name][:, :, 6] = inp[name][:, :, 1]
+    dev = to_device(inp)
+    shape = B.Shape.of(w)
+    ref = oracle.step(inp["Q_dec"], inp["Kcache"], inp["Vcache"], inp["keep"], inp["K_dec"], inp["V_dec"], w.K, w.L_q)
+    args = (shape, dev["Q_dec"], dev["Kcache"], dev["Vcache"], dev["keep"], dev["K_dec"], dev["V_dec"])
+    for S in (1, 3):
+        ws = B.alloc_workspace(shape, S)
+        folded = B.step(*args, n_splits=S, workspace=ws)
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(5)]
+        for e in ev:
+            e.record()
+        apart = B.step(*args, n_splits=S, workspace=ws, events=ev)
+        gi_ref = oracle.gather_idx(ref["ids"], inp["keep"], w.N, w.C)
+        gidx = torch.empty(gi_ref.shape, dtype=torch.int32, device="cuda")
+        exported = B.step(*args, n_splits=S, workspace=ws, gather_idx_out=gidx)
+        torch.cuda.synchronize()
+        check_exact(folded["chunk_ids"], ref["ids"])
+        check_close(folded["scores"], ref["scores"], SCORE_ABS, what="scores")
+        check_O(folded["O"], ref["O"]); check_close(folded["LSE"], ref["LSE"], LSE_ABS)
+        for other, what in ((apart, "stage events"), (exported, "gather export")):
+            assert torch.equal(folded["chunk_ids"], other["chunk_ids"]), what
+            assert torch.equal(folded["scores"].view(torch.int32), other["scores"].view(torch.int32)), what
+            assert torch.equal(folded["O"].view(torch.int16), other["O"].view(torch.int16)), what
+            assert torch.equal(folded["LSE"].view(torch.int32), other["LSE"].view(torch.int32)), what
+        check_exact(gidx, gi_ref, "gather_idx")
