@@ -102,6 +102,31 @@ score_kernel(const ScoreParams p, const __grid_constant__ CUtensorMap tmap128, c
     const int n1 = (int)min((int64_t)p.N, (int64_t)n0 + min(u_hi - u, (int64_t)kMaxChunksPerCta));
     const int bg = (int)(bgm / p.m_tiles), mt = (int)(bgm % p.m_tiles);
     const int b = bg / p.H_kv, g = bg % p.H_kv;
+    // TMA producer state of this segment; its first ST tiles go out BEFORE the Q tile is staged (every ring stage is
+    // free at a segment start: the previous segment's MMAs are complete), so the two round trips overlap
+    int pn = n0, ptt = 0;
+    auto produce = [&](int max_tiles) {
+        const uint64_t policy = l2_policy_evict_first();
+        for (; pn < n1 && max_tiles > 0; --max_tiles, ++q) {
+            const int64_t row0 = ((int64_t)bg * p.N + pn) * p.Cp;
+            const int stage = q % ST;
+            const int valid = min(kTileN, p.Cp - ptt * kTileN);
+            const bool small = valid <= 16;
+            mbar_wait(k_free(stage), ((q / ST) & 1) ^ 1);
+            mbar_arrive_expect_tx(k_full(stage), (uint32_t)(small ? 16 : 128) * D * 2);
+            const CUtensorMap *tm = small ? &tmap16 : &tmap128;
+            const int32_t row = (int32_t)(row0 + (int64_t)ptt * kTileN);
+#pragma unroll
+            for (int pnl = 0; pnl < Cfg::kPanels; ++pnl) {
+                if (p.evict_first)
+                    tma_load_2d_hint(sK(stage) + pnl * Cfg::kPanelBytes, tm, pnl * 64, row, k_full(stage), policy);
+                else
+                    tma_load_2d(sK(stage) + pnl * Cfg::kPanelBytes, tm, pnl * 64, row, k_full(stage));
+            }
+            if (++ptt == tiles_per_chunk) { ptt = 0; ++pn; }
+        }
+    };
+    if (warp == kTmaWarp && lane == 0) produce(ST);
     // Q tile (scoring rows mt*128.. of group g; row m -> head g*G + m / L_q, position m % L_q); the previous
     // segment's MMAs are complete (its softmax consumed every S tile before the barrier below was passed)
     for (int i = tid; i < kTileM * kChunksPerRow; i += kScoreThreads) {
@@ -122,28 +147,7 @@ score_kernel(const ScoreParams p, const __grid_constant__ CUtensorMap tmap128, c
 
     if (warp == kTmaWarp) {
         // =============================== TMA producer ===============================
-        if (lane == 0) {
-            const uint64_t policy = l2_policy_evict_first();
-            for (int n = n0; n < n1; ++n) {
-                const int64_t row0 = ((int64_t)bg * p.N + n) * p.Cp;
-                for (int tt = 0; tt < tiles_per_chunk; ++tt, ++q) {
-                    const int stage = q % ST;
-                    const int valid = min(kTileN, p.Cp - tt * kTileN);
-                    const bool small = valid <= 16;
-                    mbar_wait(k_free(stage), ((q / ST) & 1) ^ 1);
-                    mbar_arrive_expect_tx(k_full(stage), (uint32_t)(small ? 16 : 128) * D * 2);
-                    const CUtensorMap *tm = small ? &tmap16 : &tmap128;
-                    const int32_t row = (int32_t)(row0 + (int64_t)tt * kTileN);
-#pragma unroll
-                    for (int pn = 0; pn < Cfg::kPanels; ++pn) {
-                        if (p.evict_first)
-                            tma_load_2d_hint(sK(stage) + pn * Cfg::kPanelBytes, tm, pn * 64, row, k_full(stage), policy);
-                        else
-                            tma_load_2d(sK(stage) + pn * Cfg::kPanelBytes, tm, pn * 64, row, k_full(stage));
-                    }
-                }
-            }
-        }
+        if (lane == 0) produce(INT_MAX);
         __syncwarp();
     } else if (warp == kMmaWarp) {
         // =============================== MMA issuer ===============================
