@@ -14,6 +14,7 @@ template <int D>
 __global__ void __launch_bounds__(kCombineWarps * 32) combine_kernel(const float *__restrict__ O_part,
                                                                      const float *__restrict__ lse_part, int S, int64_t rows,
                                                                      uint16_t *__restrict__ O, float *__restrict__ LSE) {
+    constexpr int NB = 4;                          // partial rows in flight per lane (8 measured: no different)
     constexpr int V = D / 32;                      // floats per lane: 4 (d=128) or 2 (d=64)
     // launched as a programmatic dependent of the kernel that writes the partials (its launch is processed while that
     // kernel still runs): wait for that grid's completion and flush before reading them
@@ -22,8 +23,12 @@ __global__ void __launch_bounds__(kCombineWarps * 32) combine_kernel(const float
     const int64_t row = (int64_t)blockIdx.x * kCombineWarps + warp;
     if (row >= rows) return;
 
-    float big = -INFINITY;
-    for (int s = lane; s < S; s += 32) big = fmaxf(big, lse_part[(int64_t)s * rows + row]);
+    // every split's log-mass of this row in ONE round trip (lane s holds splits s and s + 32; splits beyond 64 by plain loops), the weights by
+    // shuffles, then the partial rows NB loads at a time: 1 + ceil(S / NB) dependent round trips per row, not 1 + S
+    const float x0 = lane < S ? lse_part[(int64_t)lane * rows + row] : -INFINITY;
+    const float x1 = lane + 32 < S ? lse_part[(int64_t)(lane + 32) * rows + row] : -INFINITY;
+    float big = fmaxf(x0, x1);
+    for (int sp = lane + 64; sp < S; sp += 32) big = fmaxf(big, lse_part[(int64_t)sp * rows + row]);   // (S > 64: never the library's own choice)
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) big = fmaxf(big, __shfl_xor_sync(0xffffffffu, big, o));
 
@@ -32,25 +37,44 @@ __global__ void __launch_bounds__(kCombineWarps * 32) combine_kernel(const float
     for (int i = 0; i < V; ++i) acc[i] = 0.f;
     float lse = -INFINITY;
     if (big > -INFINITY) {
-        float tot = 0.f;
-        for (int s = lane; s < S; s += 32) {
-            const float x = lse_part[(int64_t)s * rows + row];
+        float tot = (x0 > -INFINITY ? __expf(x0 - big) : 0.f) + (x1 > -INFINITY ? __expf(x1 - big) : 0.f);
+        for (int sp = lane + 64; sp < S; sp += 32) {
+            const float x = lse_part[(int64_t)sp * rows + row];
             if (x > -INFINITY) tot += __expf(x - big);
         }
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) tot += __shfl_xor_sync(0xffffffffu, tot, o);
         lse = big + __logf(tot);
-        for (int s = 0; s < S; ++s) {
-            const float x = lse_part[(int64_t)s * rows + row];         // warp-uniform broadcast load
-            if (!(x > -INFINITY)) continue;                             // empty split contributes nothing
-            const float w = __expf(x - lse);
-            const float *src = O_part + ((int64_t)s * rows + row) * D + lane * V;
-            if (V == 4) {
-                const float4 v = *reinterpret_cast<const float4 *>(src);
-                acc[0] += w * v.x; acc[1] += w * v.y; acc[V - 2] += w * v.z; acc[V - 1] += w * v.w;
-            } else {
-                const float2 v = *reinterpret_cast<const float2 *>(src);
-                acc[0] += w * v.x; acc[1] += w * v.y;
+        const float w0 = x0 > -INFINITY ? __expf(x0 - lse) : 0.f;       // an empty split contributes nothing
+        const float w1 = x1 > -INFINITY ? __expf(x1 - lse) : 0.f;
+        const float *src = O_part + row * D + lane * V;
+        for (int s0 = 0; s0 < S; s0 += NB) {
+            float v[NB][V];
+#pragma unroll
+            for (int k = 0; k < NB; ++k) {
+                const bool on = s0 + k < S;
+                const float *ptr = src + (int64_t)(on ? s0 + k : s0) * rows * D;
+                if (V == 4) {
+                    const float4 t = *reinterpret_cast<const float4 *>(ptr);
+                    v[k][0] = t.x; v[k][1] = t.y; v[k][V - 2] = t.z; v[k][V - 1] = t.w;
+                } else {
+                    const float2 t = *reinterpret_cast<const float2 *>(ptr);
+                    v[k][0] = t.x; v[k][1] = t.y;
+                }
+            }
+#pragma unroll
+            for (int k = 0; k < NB; ++k) {
+                const int sp = s0 + k;
+                float w = __shfl_sync(0xffffffffu, sp < 32 ? w0 : w1, sp & 31);
+                if (sp >= 64 && sp < S) {
+                    const float x = lse_part[(int64_t)sp * rows + row];
+                    w = x > -INFINITY ? __expf(x - lse) : 0.f;
+                }
+                if (sp >= S) w = 0.f;
+                if (w > 0.f) {                                          // (an empty split's partial row may hold anything)
+#pragma unroll
+                    for (int i = 0; i < V; ++i) acc[i] += w * v[k][i];
+                }
             }
         }
     }

@@ -73,7 +73,8 @@ def test_gather_idx_no_keep(B):
 
 
 # --------------------------------------------------------------------------- a5 combine
-@pytest.mark.parametrize("S,rows,d", [(1, 37, 128), (2, 300, 128), (4, 48, 64), (7, 1000, 128), (64, 129, 64)])
+@pytest.mark.parametrize("S,rows,d", [(1, 37, 128), (2, 300, 128), (4, 48, 64), (5, 77, 128), (7, 1000, 128), (33, 40, 128),
+                                      (64, 129, 64), (65, 33, 128), (100, 50, 64)])
 def test_lse_combine(B, S, rows, d):
     r = np.random.default_rng(S * 7 + rows)
     Op = r.standard_normal((S, rows, d)).astype(np.float32)
