@@ -22,6 +22,7 @@ namespace {
 constexpr int kScoreThreads = 320;        // 8 softmax warps (two column halves) + TMA warp + MMA warp
 constexpr int kTmaWarp = 8, kMmaWarp = 9;
 constexpr int kMaxChunksPerCta = 64;
+constexpr int kTailGroup = 4;             // one-row tails (C = 2^k: Cp = 128 t + 1) of this many consecutive chunks share a tile step
 constexpr bool kPolyShare = true;          // MUFU is co-critical with HBM here (538 M ex2 per C4 launch): offload 1/4
 
 struct ScoreParams {
@@ -63,6 +64,7 @@ score_kernel(const ScoreParams p, const __grid_constant__ CUtensorMap tmap128, c
     __shared__ uint32_t tmem_slot;
     __shared__ float s_acc[kMaxChunksPerCta * 4];
     __shared__ float s_ml[2][kTileM][2];      // column half 1's (m_ref, l) per row, double-buffered by chunk parity
+    __shared__ float s_tail[kTailGroup - 1][kTileM];   // tail logits (log2 units) of a group's later chunks, per row
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     // a dependent kernel (top-K, launched with programmatic stream serialization) may become resident beside this one;
@@ -71,6 +73,12 @@ score_kernel(const ScoreParams p, const __grid_constant__ CUtensorMap tmap128, c
     // persistent CTA: a contiguous range of the units u = ((bg * m_tiles + mt) * N + n)
     const int64_t u_lo = p.units * blockIdx.x / gridDim.x, u_hi = p.units * (blockIdx.x + 1) / gridDim.x;
     const int tiles_per_chunk = (p.Cp + kTileN - 1) / kTileN;
+    // A chunk of 128 t + 1 rows (C = 2^k plus the BOS row) ends in a one-row tile.  Such tails do not get a tile step each:
+    // the chunks of a segment form groups of kTailGroup; after the main tiles of a group's FIRST chunk one step takes the
+    // tail rows of all its chunks (a 16-row TMA box each, side by side in one ring stage, one MMA of N = 16 g) -- the
+    // first chunk folds its tail in as before, the others start from theirs.  4 + 1/kTailGroup steps per chunk, not 5.
+    const bool tail_groups = tiles_per_chunk > 1 && p.Cp - (tiles_per_chunk - 1) * kTileN == 1;
+    const int main_tiles = tail_groups ? tiles_per_chunk - 1 : tiles_per_chunk;
 
     const uint32_t bar0 = smem_u32(&bars[0]);
     auto k_full = [&](int s) { return bar0 + 8u * s; };
@@ -110,20 +118,34 @@ score_kernel(const ScoreParams p, const __grid_constant__ CUtensorMap tmap128, c
         for (; pn < n1 && max_tiles > 0; --max_tiles, ++q) {
             const int64_t row0 = ((int64_t)bg * p.N + pn) * p.Cp;
             const int stage = q % ST;
-            const int valid = min(kTileN, p.Cp - ptt * kTileN);
-            const bool small = valid <= 16;
             mbar_wait(k_free(stage), ((q / ST) & 1) ^ 1);
-            mbar_arrive_expect_tx(k_full(stage), (uint32_t)(small ? 16 : 128) * D * 2);
-            const CUtensorMap *tm = small ? &tmap16 : &tmap128;
-            const int32_t row = (int32_t)(row0 + (int64_t)ptt * kTileN);
+            if (ptt < main_tiles) {
+                const int valid = min(kTileN, p.Cp - ptt * kTileN);
+                const bool small = valid <= 16;
+                mbar_arrive_expect_tx(k_full(stage), (uint32_t)(small ? 16 : 128) * D * 2);
+                const CUtensorMap *tm = small ? &tmap16 : &tmap128;
+                const int32_t row = (int32_t)(row0 + (int64_t)ptt * kTileN);
 #pragma unroll
-            for (int pnl = 0; pnl < Cfg::kPanels; ++pnl) {
-                if (p.evict_first)
-                    tma_load_2d_hint(sK(stage) + pnl * Cfg::kPanelBytes, tm, pnl * 64, row, k_full(stage), policy);
-                else
-                    tma_load_2d(sK(stage) + pnl * Cfg::kPanelBytes, tm, pnl * 64, row, k_full(stage));
+                for (int pnl = 0; pnl < Cfg::kPanels; ++pnl) {
+                    if (p.evict_first)
+                        tma_load_2d_hint(sK(stage) + pnl * Cfg::kPanelBytes, tm, pnl * 64, row, k_full(stage), policy);
+                    else
+                        tma_load_2d(sK(stage) + pnl * Cfg::kPanelBytes, tm, pnl * 64, row, k_full(stage));
+                }
+            } else {
+                // the group's tail rows: chunk pn + k's last row (and the 15 rows behind it) at tile rows 16 k ..
+                const int g = min(kTailGroup, n1 - pn);
+                mbar_arrive_expect_tx(k_full(stage), (uint32_t)(16 * g) * D * 2);
+                for (int k = 0; k < g; ++k) {
+                    const int32_t row = (int32_t)(row0 + (int64_t)k * p.Cp + (int64_t)main_tiles * kTileN);
+#pragma unroll
+                    for (int pnl = 0; pnl < Cfg::kPanels; ++pnl)
+                        tma_load_2d(sK(stage) + pnl * Cfg::kPanelBytes + (uint32_t)k * 2048u, &tmap16, pnl * 64, row, k_full(stage));
+                }
             }
-            if (++ptt == tiles_per_chunk) { ptt = 0; ++pn; }
+            // next step: the main tiles of every chunk, then -- behind a group's first chunk -- the group's tails
+            const bool leader = tail_groups && (pn - n0) % kTailGroup == 0;
+            if (++ptt == main_tiles + (leader ? 1 : 0)) { ptt = 0; ++pn; }
         }
     };
     if (warp == kTmaWarp && lane == 0) produce(ST);
@@ -153,10 +175,11 @@ score_kernel(const ScoreParams p, const __grid_constant__ CUtensorMap tmap128, c
         // =============================== MMA issuer ===============================
         if (lane == 0) {
             for (int n = n0; n < n1; ++n) {
-                for (int tt = 0; tt < tiles_per_chunk; ++tt, ++q) {
+                const bool leader = tail_groups && (n - n0) % kTailGroup == 0;
+                for (int tt = 0; tt < main_tiles + (leader ? 1 : 0); ++tt, ++q) {
                     const int stage = q % ST, buf = q & 1;
                     const int valid = min(kTileN, p.Cp - tt * kTileN);
-                    const uint32_t n_mma = (uint32_t)(valid + 15) & ~15u;
+                    const uint32_t n_mma = tt < main_tiles ? (uint32_t)(valid + 15) & ~15u : 16u * (uint32_t)min(kTailGroup, n1 - n);
                     mbar_wait(k_full(stage), (q / ST) & 1);
                     mbar_wait(s_free(buf), ((q >> 1) & 1) ^ 1);
                     tc_fence_after();
@@ -186,6 +209,12 @@ score_kernel(const ScoreParams p, const __grid_constant__ CUtensorMap tmap128, c
         constexpr float kSumLimit = 8192.f;
         for (int n = n0; n < n1; ++n) {
             float m_ref = -INFINITY, l = 0.f;
+            const int in_group = tail_groups ? (n - n0) % kTailGroup : 0;
+            const bool leader = tail_groups && in_group == 0;
+            if (in_group > 0 && half == 0) {          // the chunk starts from its tail row, taken in the group's tail step
+                m_ref = s_tail[in_group - 1][row];    // (written by this very thread)
+                l = 1.f;
+            }
             // sum over 32 columns of 2^(c2*x - m_ref): packed f32x2 arithmetic, exponentials on the MUFU pipe
             auto block_sum = [&](const uint32_t(&v)[32]) {
                 const uint64_t c2v = pack_f32x2(p.c2, p.c2), mv = pack_f32x2(-m_ref, -m_ref);
@@ -209,7 +238,7 @@ score_kernel(const ScoreParams p, const __grid_constant__ CUtensorMap tmap128, c
                 unpack_f32x2(acc1, s2, s3);
                 return (s0 + s1) + (s2 + s3);
             };
-            for (int tt = 0; tt < tiles_per_chunk; ++tt, ++q) {
+            for (int tt = 0; tt < main_tiles + (leader ? 1 : 0); ++tt, ++q) {
                 const int buf = q & 1;
                 const int valid = min(kTileN, p.Cp - tt * kTileN);
                 const uint32_t tS = tmem + 128u * buf + lane_base;
@@ -229,7 +258,7 @@ score_kernel(const ScoreParams p, const __grid_constant__ CUtensorMap tmap128, c
                             for (int e = 0; e < 32; ++e)
                                 mx[e & 3] = fmaxf(mx[e & 3], fmaxf(__uint_as_float(va[e]), __uint_as_float(vb[e])));
                             const float tm2 = fmaxf(fmaxf(mx[0], mx[1]), fmaxf(mx[2], mx[3])) * p.c2;
-                            if (tt == 0) {
+                            if (tt == 0 && !(l > 0.f)) {
                                 m_ref = tm2;
                             } else {                      // raise the reference by whole octaves (exact rescale of l)
                                 const float up = fmaxf(ceilf(tm2 - m_ref), 0.f);
@@ -256,7 +285,16 @@ score_kernel(const ScoreParams p, const __grid_constant__ CUtensorMap tmap128, c
                     // threads of column half 0 alone
                     if (half == 0) {
                         const uint32_t xv = tmem_ld1(tS);
+                        uint32_t xg[kTailGroup - 1];
+                        if (leader) {                     // the tails of the group's other chunks sit 16 columns apart
+#pragma unroll
+                            for (int k = 0; k < kTailGroup - 1; ++k) xg[k] = tmem_ld1(tS + 16u * (k + 1));
+                        }
                         tmem_wait_ld();
+                        if (leader) {
+#pragma unroll
+                            for (int k = 0; k < kTailGroup - 1; ++k) s_tail[k][row] = __uint_as_float(xg[k]) * p.c2;
+                        }
                         const float x2 = __uint_as_float(xv) * p.c2;
                         tc_fence_before();
                         mbar_arrive(s_free(buf));

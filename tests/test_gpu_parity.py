@@ -448,6 +448,42 @@ def test_step_explicit_scale_and_strict_rows(B):
     dict(B=1, H=12, H_kv=4, d=64, N=2000, C=12, K=5, L_q=100, L_d=4),  # GQA G = 3: 300 scoring rows = 3 M tiles, 81 units per CTA
 ])
 def test_scores_long_cta_runs(B, kw):
+    _scores_case(B, kw)
+
+
+@pytest.mark.parametrize("kw", [
+    dict(B=5, H=8, H_kv=8, d=64, N=512, C=128, K=4, L_q=16, L_d=8),     # Cp = 129: one main tile + a one-row tail; 69 chunks per CTA:
+                                                                        # tail groups of 4 restart at every 64-chunk segment
+    dict(B=1, H=4, H_kv=4, d=128, N=5, C=256, K=2, L_q=40, L_d=8),      # 20 chunks on 20 CTAs: every group is a single chunk
+    dict(B=1, H=2, H_kv=2, d=128, N=301, C=128, K=3, L_q=128, L_d=8),   # 602 chunks / 296 CTAs: runs of 2-3 chunks, groups cut short
+    dict(B=1, H=6, H_kv=2, d=64, N=23, C=384, K=3, L_q=60, L_d=4),      # GQA G = 3: 180 rows = 2 M tiles (partial M tile), Cp = 385
+    dict(B=5, H=8, H_kv=8, d=128, N=64, C=128, K=4, L_q=32, L_d=8),     # 2560 chunks / 296 CTAs: runs of 8-9 = groups of 4, 4, (1)
+    dict(B=1, H=1, H_kv=1, d=128, N=1, C=1024, K=1, L_q=16, L_d=8),     # a single chunk
+])
+def test_scores_one_row_tails_in_groups(B, kw):
+    """Chunks of 128 t + 1 rows (C = 2^k): the score kernel takes the one-row tails of up to four consecutive chunks of a
+    CTA's run in ONE tile step behind the first of them; the later chunks start their running (max, sum) from that
+    row.  Runs that start / end inside a group, single-chunk runs, segment restarts, GQA."""
+    _scores_case(B, kw)
+
+
+@pytest.mark.parametrize("gain", [0.0, 1.0, 40.0])
+def test_scores_tail_row_dominates_or_vanishes(B, gain):
+    """The last cached row of every second chunk scaled by `gain` along the mean query: with 40 its logit sits far above
+    the chunk's other 256 (the chunk's running max then starts from the tail row and never rises), with 0 it is an
+    average key; both through the grouped-tail path (Cp = 257) and against the oracle."""
+    w, inp = _inputs("tiny", B=2, H=4, H_kv=4, d=128, N=11, C=256, K=2, L_q=48, L_d=8)
+    Kc = W.bf16_bits_to_f32(inp["Kcache"]).copy()
+    qm = W.bf16_bits_to_f32(inp["Q_dec"])[:, :, :w.L_q].mean(axis=2)           # [B, H, d] (H = H_kv here)
+    Kc[:, :, ::2, w.C, :] = gain * qm[:, :, None, :]
+    inp["Kcache"] = W.f32_to_bf16_bits(Kc)
+    shape = B.Shape.of(w)
+    got = B.score_chunks(shape, dev_bf16(inp["Q_dec"]), dev_bf16(inp["Kcache"]))
+    ref = oracle.scores(inp["Q_dec"], inp["Kcache"], w.L_q)
+    check_close(got, ref, SCORE_ABS * max(1.0, float(np.abs(ref).max()) / 100.0), what="scores (tail rows)")
+
+
+def _scores_case(B, kw):
     w, inp = _inputs("tiny", **kw)
     shape = B.Shape.of(w)
     got = B.score_chunks(shape, dev_bf16(inp["Q_dec"]), dev_bf16(inp["Kcache"]))
