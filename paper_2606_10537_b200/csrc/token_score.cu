@@ -207,6 +207,12 @@ token_score_kernel(const TokParams p, const __grid_constant__ CUtensorMap tmap12
                 const uint32_t tS = tmem + 128u * buf + lane_base;
                 mbar_wait(s_ready(buf), (q >> 1) & 1);
                 tc_fence_after();
+                if ((warp & 3) * 32 >= valid) {           // ragged tail tile: none of this warp's 32 slots is a cache row
+                    tc_fence_before();
+                    mbar_arrive(s_free(buf));
+                    asm volatile("bar.sync %0, 64;" ::"r"(pair_bar) : "memory");
+                    continue;
+                }
                 uint32_t va[32], vb[32];
                 tmem_ld32(tS, va);
                 tmem_wait_ld();
