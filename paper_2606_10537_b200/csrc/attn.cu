@@ -39,6 +39,7 @@ constexpr int kAttnThreads = 2 * kSoftmaxThreads + kProducerThreads + 128;     /
 // register budgets after the roles part ways (setmaxnreg; 256 * 176 + 128 * 104 + 128 * 56 = 65536)
 constexpr int kSoftmaxRegs = 176, kProducerRegs = 104, kOtherRegs = 56;
 constexpr int kInvalidRow = INT32_MIN;
+static_assert(PDLLM_FOLD_MAX_N == 128, "four producer warps rank 32 chunks each; ids are kept as bytes");
 constexpr int kFoldMaxN = PDLLM_FOLD_MAX_N;              // top-K is folded into the kernel up to this many chunks
 constexpr float kRescaleThreshold = 8.0f;                 // log2 units: P stays <= 2^8 between reference-max updates
 
@@ -167,7 +168,8 @@ attn_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tm_kp, const
     __shared__ uint64_t bars[BAR_KV + 2 * (ST + 1)];
     __shared__ uint32_t tmem_slot;
     __shared__ int32_t s_items[4];                        // the CTA's next work items (ring, published by the producers)
-    __shared__ int32_t s_ids[64];                         // folded top-K: the current item's chunk ids
+    __shared__ uint8_t s_ids[64];                         // folded top-K: the current item's chunk ids (< kFoldMaxN <= 256)
+    __shared__ uint32_t s_mask[4];                        // folded top-K: selection bitmask per producer warp
     __shared__ float s_ml[kSoftmaxThreads][3];            // single items: stream 1's (m_ref, l, O scale) for the in-CTA merge
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -285,49 +287,51 @@ attn_kernel(const AttnParams p, const __grid_constant__ CUtensorMap tm_kp, const
             // the group's K <= 64 chunk ids live in two registers per lane (lane l: ids[l], ids[l + 32])
             int ids_lo = 0, ids_hi = 0;
             if (p.fold_scores) {
-                // a2 (R6) inside the kernel: producer warp 0 ranks the group's N <= 128 scores -- rank = number of
+                // a2 (R6) inside the kernel: the producer warps rank the group's N <= 128 scores -- rank = number of
                 // chunks ahead in the (score descending, index ascending) order; the K chunks of rank < K are the selection
                 // -- and lists them in ascending index order.  Every item of the group arrives at the same list.
-                if (pw == 0) {
-                    float v[kFoldMaxN / 32];
-                    int rank[kFoldMaxN / 32];
+                // All four producer warps hold the scores (lane l: chunks l, l + 32, l + 64, l + 96); warp w ranks chunks
+                // 32 w .. 32 w + 31 against all of them by shuffle broadcasts.
+                float v[kFoldMaxN / 32];
 #pragma unroll
-                    for (int r = 0; r < kFoldMaxN / 32; ++r) {
-                        const int idx = r * 32 + lane;
-                        float x = -INFINITY;
-                        if (idx < p.N) {
-                            x = 0.f;
-                            for (int mt = 0; mt < p.fold_m_tiles; ++mt) x += p.fold_scores[mt * p.fold_stride + bg * p.N + idx];
-                            if (p.fold_scores_out && it.q0 == 0 && it.split == 0) p.fold_scores_out[bg * p.N + idx] = x;
-                            if (x != x) x = -INFINITY;        // NaN counts as -inf
-                        }
-                        v[r] = x;
-                        rank[r] = 0;
+                for (int r = 0; r < kFoldMaxN / 32; ++r) {
+                    const int idx = r * 32 + lane;
+                    float x = -INFINITY;
+                    if (idx < p.N) {
+                        x = 0.f;
+                        for (int mt = 0; mt < p.fold_m_tiles; ++mt) x += p.fold_scores[mt * p.fold_stride + bg * p.N + idx];
+                        if (p.fold_scores_out && pw == r && it.q0 == 0 && it.split == 0) p.fold_scores_out[bg * p.N + idx] = x;
+                        if (x != x) x = -INFINITY;            // NaN counts as -inf
                     }
+                    v[r] = x;
+                }
+                const int my_idx = pw * 32 + lane;
+                const float mine = pw == 0 ? v[0] : pw == 1 ? v[1] : pw == 2 ? v[2] : v[3];
+                int rank = 0;
+                // (eight broadcasts in flight per trip of a rolled loop: the code stays small -- it runs cold once per launch)
+#pragma unroll 1
+                for (int r2 = 0; r2 * 32 < p.N; ++r2) {
+                    const float vr = r2 == 0 ? v[0] : r2 == 1 ? v[1] : r2 == 2 ? v[2] : v[3];
+#pragma unroll 1
+                    for (int l0 = 0; l0 < 32; l0 += 8) {
 #pragma unroll
-                    for (int r2 = 0; r2 < kFoldMaxN / 32; ++r2) {
-                        if (r2 * 32 >= p.N) break;
-                        for (int l2 = 0; l2 < 32 && r2 * 32 + l2 < p.N; ++l2) {
-                            const float o = __shfl_sync(0xffffffffu, v[r2], l2);
-                            const int idx2 = r2 * 32 + l2;
-#pragma unroll
-                            for (int r = 0; r < kFoldMaxN / 32; ++r)
-                                if (r * 32 < p.N) rank[r] += (o > v[r] || (o == v[r] && idx2 < r * 32 + lane)) ? 1 : 0;
+                        for (int l2 = 0; l2 < 8; ++l2) {      // (chunks past N hold -inf behind every real index: never ahead)
+                            const float o = __shfl_sync(0xffffffffu, vr, l0 + l2);
+                            rank += (o > mine || (o == mine && r2 * 32 + l0 + l2 < my_idx)) ? 1 : 0;
                         }
                     }
-                    int base = 0;
+                }
+                const bool sel = my_idx < p.N && rank < p.K;
+                const uint32_t sel_mask = __ballot_sync(0xffffffffu, sel);
+                if (lane == 0) s_mask[pw] = sel_mask;
+                asm volatile("bar.sync 1, 128;" ::: "memory");
+                if (sel) {
+                    int pos = __popc(sel_mask & ((1u << lane) - 1u));
 #pragma unroll
-                    for (int r = 0; r < kFoldMaxN / 32; ++r) {
-                        const int idx = r * 32 + lane;
-                        const bool sel = idx < p.N && rank[r] < p.K;
-                        const uint32_t m = __ballot_sync(0xffffffffu, sel);
-                        if (sel) {
-                            const int pos = base + __popc(m & ((1u << lane) - 1u));
-                            s_ids[pos] = idx;
-                            if (it.q0 == 0 && it.split == 0) p.fold_ids_out[bg * p.K + pos] = idx;
-                        }
-                        base += __popc(m);
-                    }
+                    for (int w2 = 0; w2 < 3; ++w2)
+                        if (w2 < pw) pos += __popc(s_mask[w2]);
+                    s_ids[pos] = (uint8_t)my_idx;
+                    if (it.q0 == 0 && it.split == 0) p.fold_ids_out[bg * p.K + pos] = my_idx;
                 }
                 asm volatile("bar.sync 1, 128;" ::: "memory");
                 ids_lo = lane < p.K ? s_ids[lane] : 0;
