@@ -45,8 +45,8 @@ SPEC_PEAKS = {"hbm_gbs": 8000.0, "bf16_tflops": 2250.0}      # the peaks BASELIN
 # (workload, kernel); None where no capture exists for that pair.
 NCU_TRAFFIC_SOURCE = "profiles/r2_ncu_full.md (ncu --set full capture of these kernels; not measured in this run)"
 NCU_TRAFFIC_BYTES = {
-    ("sparse32k", "score_kernel"): 1081.249e6 + 3.572480e6,
-    ("sparse32k", "attn_kernel"): 148.781e6 + 6.031872e6,
+    ("sparse32k", "score_kernel"): 1081.614e6 + 3.672064e6,
+    ("sparse32k", "attn_kernel"): 154.260e6 + 6.714112e6,
 }
 
 
