@@ -66,7 +66,8 @@ typedef enum {
     PDLLM_ERR_WORKSPACE = -4,   /* workspace_bytes smaller than pdllm_workspace_bytes() */
     PDLLM_ERR_UNSUPPORTED = -5, /* valid request that this build does not implement */
     PDLLM_ERR_CUDA = -6,        /* a CUDA runtime / driver call or a launch failed */
-    PDLLM_ERR_DATA = -7         /* PDLLM_DEBUG_VALIDATE=1 only: a device-side index list is malformed */
+    PDLLM_ERR_DATA = -7,        /* PDLLM_DEBUG_VALIDATE=1 only: a device-side index list is malformed */
+    PDLLM_ERR_SCRATCH_LIMIT = -8 /* pdllm_sparse_attn_noalloc: the request needs more than PDLLM_NOALLOC_SCRATCH_BYTES */
 } pdllm_status;
 
 /* Shapes shared by all calls (S8 symbols).
@@ -342,6 +343,37 @@ int pdllm_select_topb(const pdllm_shape *shape, const float *token_scores, int32
 int pdllm_prefill_attn(const pdllm_dense_shape *shape, const void *Q, const void *K, const void *V,
                        int32_t n_splits, void *O, float *LSE, void *workspace,
                        size_t workspace_bytes, pdllm_stream_t stream);
+
+/* ---- a3 + a4 + a5 without a caller workspace: the call that allocates nothing -----
+ * pdllm_sparse_attn (same arguments, same kernels, same results)
+ * for callers that cannot call cudaMalloc: code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid allocation.  The scratch the path needs (the
+ * persistent kernel's work-item counter; the fp32 Split-S partials when more than
+ * one split runs) lives in ONE file-scope device array of
+ * PDLLM_NOALLOC_SCRATCH_BYTES inside the library: every GPU that loads the library
+ * holds those bytes until the process exits; the call itself calls no cudaMalloc,
+ * cudaFree or allocating library routine.  Inputs and outputs are still the
+ * caller's.
+ *   limit     an explicit n_splits whose pdllm_workspace_bytes(shape, n_splits, 0)
+ *             exceeds PDLLM_NOALLOC_SCRATCH_BYTES returns PDLLM_ERR_SCRATCH_LIMIT with
+ *             nothing enqueued; n_splits == 0 takes the auto choice, lowered to the
+ *             largest split count the array holds (one split always fits).  The
+ *             limit covers every named workload (C3 at 3 splits: 16.6 MB).
+ *   sharing   every call on a device uses the same array, which keeps the previous
+ *             call's contents; what must start at zero (the work-item counter) is
+ *             cleared on `stream` by the call, the partials are written in full
+ *             before they are read.  Calls that OVERLAP on one GPU (different
+ *             streams, or several host threads) race on the array: serialise them,
+ *             or use pdllm_sparse_attn with a workspace per stream.
+ *   set-up    the array's device address is looked up once per device
+ *             (cudaGetSymbolAddress with the caller's device current) on the first
+ *             call there; make that first call outside a stream capture.          */
+#define PDLLM_NOALLOC_SCRATCH_BYTES (32u << 20)
+int pdllm_sparse_attn_noalloc(const pdllm_shape *shape, const void *Q_dec, const void *Kcache,
+                              const void *Vcache, const int32_t *chunk_ids,
+                              const int32_t *token_keep_idx, const void *K_dec, const void *V_dec,
+                              int32_t n_splits, void *O, float *LSE, int32_t *gather_idx_out,
+                              pdllm_stream_t stream);
 
 #ifdef __cplusplus
 }

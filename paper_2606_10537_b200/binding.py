@@ -26,7 +26,11 @@ EXPORTS = [
     "pdllm_compact_kv", "pdllm_dense_auto_splits", "pdllm_dense_workspace_bytes", "pdllm_static_attn",
     "pdllm_pool_keys", "pdllm_score_chunks_pooled", "pdllm_prefill_attn",
     "pdllm_score_tokens_workspace_bytes", "pdllm_score_tokens", "pdllm_select_topb",
+    # the call that allocates nothing (scratch in a fixed device array inside the library)
+    "pdllm_sparse_attn_noalloc",
 ]
+NOALLOC_SCRATCH_BYTES = 32 << 20        # include/pdllm.h PDLLM_NOALLOC_SCRATCH_BYTES
+ERR_SCRATCH_LIMIT = -8                  # include/pdllm.h PDLLM_ERR_SCRATCH_LIMIT
 
 
 class PdllmShape(ctypes.Structure):
@@ -123,6 +127,7 @@ def lib() -> ctypes.CDLL:
     L.pdllm_select_topk.argtypes = [shp, vp, vp, vp]
     L.pdllm_gather_idx.argtypes = [shp, vp, vp, vp, vp]
     L.pdllm_sparse_attn.argtypes = [shp, vp, vp, vp, vp, vp, vp, vp, i32, vp, vp, vp, vp, sz, vp]
+    L.pdllm_sparse_attn_noalloc.argtypes = [shp, vp, vp, vp, vp, vp, vp, vp, i32, vp, vp, vp, vp]
     L.pdllm_lse_combine.argtypes = [vp, vp, i32, i64, i32, vp, vp, vp]
     L.pdllm_step.argtypes = [shp, vp, vp, vp, vp, vp, vp, i32, vp, vp, vp, vp, vp, vp, sz, vp]
     L.pdllm_step_profiled.argtypes = [shp, vp, vp, vp, vp, vp, vp, i32, vp, vp, vp, vp, vp, vp, sz,
@@ -149,6 +154,7 @@ def lib() -> ctypes.CDLL:
     for n in ("pdllm_score_chunks", "pdllm_select_topk", "pdllm_gather_idx", "pdllm_sparse_attn", "pdllm_lse_combine",
               "pdllm_step", "pdllm_step_profiled", "pdllm_step_host"):
         getattr(L, n).restype = ctypes.c_int
+    L.pdllm_sparse_attn_noalloc.restype = ctypes.c_int
     _lib = L
     return L
 
@@ -242,6 +248,17 @@ def sparse_attn(shape: Shape, Q_dec, Kcache, Vcache, chunk_ids, token_keep_idx, 
     _check(lib().pdllm_sparse_attn(ctypes.byref(shape.c()), _ptr(Q_dec), _ptr(Kcache), _ptr(Vcache), _ptr(chunk_ids),
                                    _ptr(token_keep_idx), _ptr(K_dec), _ptr(V_dec), n_splits, _ptr(O), _ptr(LSE),
                                    _ptr(gather_idx_out), _ptr(workspace), workspace.numel(), _stream(stream)))
+    return O, LSE
+
+
+def sparse_attn_noalloc(shape: Shape, Q_dec, Kcache, Vcache, chunk_ids, token_keep_idx, K_dec, V_dec, O, LSE, n_splits=0,
+                        gather_idx_out=None, stream=None):
+    """pdllm_sparse_attn without a workspace: the scratch is a fixed device array inside the library
+    (NOALLOC_SCRATCH_BYTES); nothing is allocated here either -- O and LSE are the caller's.  Calls that overlap on one
+    GPU race on that array."""
+    _check(lib().pdllm_sparse_attn_noalloc(ctypes.byref(shape.c()), _ptr(Q_dec), _ptr(Kcache), _ptr(Vcache),
+                                           _ptr(chunk_ids), _ptr(token_keep_idx), _ptr(K_dec), _ptr(V_dec), n_splits,
+                                           _ptr(O), _ptr(LSE), _ptr(gather_idx_out), _stream(stream)))
     return O, LSE
 
 

@@ -17,7 +17,7 @@ from pathlib import Path
 PKG = Path(__file__).resolve().parent
 CSRC = PKG / "csrc"
 LIB = PKG / "libpdllm.so"
-SOURCES = ["pdllm_api.cu", "select.cu", "combine.cu", "score.cu", "attn.cu", "static_cache.cu", "token_score.cu"]
+SOURCES = ["pdllm_api.cu", "select.cu", "combine.cu", "score.cu", "attn.cu", "static_cache.cu", "token_score.cu", "noalloc.cu"]
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 
 

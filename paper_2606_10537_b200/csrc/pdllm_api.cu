@@ -175,6 +175,7 @@ const char *pdllm_strerror(int status) {
         case PDLLM_ERR_UNSUPPORTED: return "unsupported request";
         case PDLLM_ERR_CUDA: return "CUDA call or launch failed";
         case PDLLM_ERR_DATA: return "PDLLM_DEBUG_VALIDATE: a chunk id or token-keep list on the device is malformed";
+        case PDLLM_ERR_SCRATCH_LIMIT: return "pdllm_sparse_attn_noalloc: the request needs more scratch than PDLLM_NOALLOC_SCRATCH_BYTES";
         default: return "unknown pdllm status";
     }
 }
