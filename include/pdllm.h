@@ -365,6 +365,9 @@ int pdllm_prefill_attn(const pdllm_dense_shape *shape, const void *Q, const void
  *             before they are read.  Calls that OVERLAP on one GPU (different
  *             streams, or several host threads) race on the array: serialise them,
  *             or use pdllm_sparse_attn with a workspace per stream.
+ *   debug     PDLLM_DEBUG_VALIDATE=1 makes pdllm_sparse_attn allocate a 4-byte flag
+ *             and synchronise; under that switch this call returns
+ *             PDLLM_ERR_UNSUPPORTED (debug with pdllm_sparse_attn instead).
  *   set-up    the array's device address is looked up once per device
  *             (cudaGetSymbolAddress with the caller's device current) on the first
  *             call there; make that first call outside a stream capture.          */

@@ -10,6 +10,8 @@
 // GPU can reach host memory, silently uses the wrong memory.  The device address comes from cudaGetSymbolAddress, asked
 // once per device with that device current, and is what the kernels get.
 #include <atomic>
+#include <cstdlib>
+#include <cstring>
 
 #include "pdllm_internal.h"
 
@@ -52,6 +54,10 @@ extern "C" int pdllm_sparse_attn_noalloc(const pdllm_shape *shape, const void *Q
                                          pdllm_stream_t stream) {
     if (!shape) return PDLLM_ERR_NULL;
     if (n_splits < 0) return PDLLM_ERR_SHAPE;
+    // the debug switch (include/pdllm.h, "DEBUG SWITCH") makes pdllm_sparse_attn allocate a 4-byte flag and synchronise
+    // the stream: not something this entry point may do, so it refuses to run under it rather than skip the check
+    if (const char *e = std::getenv("PDLLM_DEBUG_VALIDATE"))
+        if (e[0] != '\0' && std::strcmp(e, "0") != 0) return PDLLM_ERR_UNSUPPORTED;
     // an explicit split count whose partials do not fit the fixed array is refused before anything touches the device;
     // n_splits == 0 cannot overflow it: pdllm_sparse_attn then takes the largest split count the scratch holds
     if (n_splits > 0) {

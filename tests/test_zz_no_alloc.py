@@ -34,6 +34,21 @@ def test_limit_matches_the_header_and_oversized_requests_are_refused():
     assert lib.pdllm_workspace_bytes(ctypes.byref(shape.c()), 1, 148) <= B.NOALLOC_SCRATCH_BYTES   # one split always fits
 
 
+def test_noalloc_refuses_to_run_under_the_debug_switch(monkeypatch):
+    """PDLLM_DEBUG_VALIDATE=1 makes the workspace path allocate a flag and synchronise; the call that must not allocate
+    says so (host-side, before anything reaches a device) instead of skipping the check silently."""
+    lib = B.lib()
+    shape = B.Shape.of(W.CONFIGS["tiny"])
+    monkeypatch.setenv("PDLLM_DEBUG_VALIDATE", "1")
+    rc = lib.pdllm_sparse_attn_noalloc(ctypes.byref(shape.c()), None, None, None, None, None, None, None, 1, None, None,
+                                       None, None)
+    assert rc == -5 and b"unsupported" in lib.pdllm_strerror(rc)
+    monkeypatch.setenv("PDLLM_DEBUG_VALIDATE", "0")
+    rc = lib.pdllm_sparse_attn_noalloc(ctypes.byref(shape.c()), None, None, None, None, None, None, None, 1 << 20, None,
+                                       None, None, None)
+    assert rc != -5                                       # (an absurd split count: refused for its size or shape, not the switch)
+
+
 def _case(w, S):
     inp = W.make_inputs(w)
     dev = to_device(inp)
