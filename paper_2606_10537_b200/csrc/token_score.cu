@@ -11,7 +11,7 @@
 // halves, as in score.cu); the per-column subtrahend ell comes from shared memory as broadcast 128-bit loads; a quarter
 // of the exponentials run as the FMA-pipe polynomial.  HBM-bound at MHA shapes like the chunk-score kernel.
 // topb_kernel: one CTA per chunk, MSB-first radix select on order-preserving integer keys, ties to the lower slot,
-// ascending emission, slot 0 (BOS) always kept.
+// ascending emission, slot 0 (BOS) always kept; topb_warp_kernel: one warp per chunk (C <= 1024, many chunks).
 #include <cuda.h>
 
 #include "pdllm_internal.h"
@@ -400,8 +400,74 @@ cudaError_t launch_token_scores(const Dims &s, const void *Q, int64_t q_batch_st
 
 int topb_max_cp() { return kTopbMaxCp; }
 
+// Chunks of up to 32 R + 1 slots: one WARP per chunk, the keys of slots 1..C in registers (lane l: slots 1 + l, 33 + l, ...).
+// The threshold T = the (Bk-1)-th largest key is built bit by bit from the top (T |= bit whenever at least Bk-1 keys are
+// >= the candidate: 32 rounds of R compares and one warp reduction), then one ordered pass emits the kept slots ascending
+// with ballots and popcount prefixes.  No shared memory, no block barriers.  The search stops as soon as exactly Bk-1 keys
+// lie at or above the candidate (distinct scores: after ~20 of the 32 rounds).
+constexpr int kTopbWarps = 8;
+
+template <int R>
+__global__ void __launch_bounds__(kTopbWarps * 32) topb_warp_kernel(const float *__restrict__ e, int32_t *__restrict__ keep,
+                                                                    int chunks, int Cp, int Bk) {
+    const int lane = threadIdx.x & 31;
+    const int chunk = blockIdx.x * kTopbWarps + (threadIdx.x >> 5);
+    if (chunk >= chunks) return;
+    const float *src = e + (int64_t)chunk * Cp;
+    int32_t *dst = keep + (int64_t)chunk * Bk;
+    uint32_t key[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        const int j = 1 + r * 32 + lane;
+        key[r] = j < Cp ? order_key(__ldg(src + j)) : 0u;         // 0 is below every real key (order_key(-inf) = 0x007fffff)
+    }
+    if (lane == 0) dst[0] = 0;                                    // BOS is always kept (R7)
+    const int want = Bk - 1;
+    if (want == 0) return;
+    uint32_t T = 0u;
+#pragma unroll 1
+    for (int bit = 31; bit >= 0; --bit) {
+        const uint32_t cand = T | (1u << bit);
+        int cnt = 0;
+#pragma unroll
+        for (int r = 0; r < R; ++r) cnt += key[r] >= cand ? 1 : 0;
+        const int c = (int)__reduce_add_sync(0xffffffffu, (unsigned)cnt);
+        if (c >= want) {
+            T = cand;
+            if (c == want) break;             // exactly the keys >= T: the lower bits cannot change the selection
+        }
+    }
+    int above = 0;
+#pragma unroll
+    for (int r = 0; r < R; ++r) above += key[r] > T ? 1 : 0;
+    const int need_eq = want - (int)__reduce_add_sync(0xffffffffu, (unsigned)above);   // keys equal to T to take, lowest slots first
+    const uint32_t lt = (1u << lane) - 1u;
+    int out = 1, eq_seen = 0;
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        const int j = 1 + r * 32 + lane;
+        const bool in = j < Cp;
+        const bool eq = in && key[r] == T;
+        const uint32_t eq_mask = __ballot_sync(0xffffffffu, eq);
+        const bool sel = in && (key[r] > T || (eq && eq_seen + __popc(eq_mask & lt) < need_eq));
+        const uint32_t sel_mask = __ballot_sync(0xffffffffu, sel);
+        if (sel) dst[out + __popc(sel_mask & lt)] = j;
+        out += __popc(sel_mask);
+        eq_seen += __popc(eq_mask);
+    }
+}
+
 cudaError_t launch_topb(const Dims &s, const float *token_scores, int32_t *keep, cudaStream_t st) {
     const unsigned chunks = (unsigned)((int64_t)s.B * s.H_kv * s.N);
+    // one warp per chunk pays when there are warps enough to fill the GPU (C4: 8192 chunks, 53 -> 17 us); with few chunks
+    // the CTA-per-chunk kernel below has more threads on each of them
+    if (s.Cp - 1 <= 32 * 32 && chunks >= 1024u) {
+        const unsigned grid = (chunks + kTopbWarps - 1) / kTopbWarps;
+        if (s.Cp - 1 <= 32 * 4) topb_warp_kernel<4><<<grid, kTopbWarps * 32, 0, st>>>(token_scores, keep, (int)chunks, s.Cp, s.Bk);
+        else if (s.Cp - 1 <= 32 * 16) topb_warp_kernel<16><<<grid, kTopbWarps * 32, 0, st>>>(token_scores, keep, (int)chunks, s.Cp, s.Bk);
+        else topb_warp_kernel<32><<<grid, kTopbWarps * 32, 0, st>>>(token_scores, keep, (int)chunks, s.Cp, s.Bk);
+        return cudaGetLastError();
+    }
     const size_t smem = (size_t)s.Cp * sizeof(uint32_t);
     topb_kernel<<<chunks, kTopbThreads, smem, st>>>(token_scores, keep, s.Cp, s.Bk);
     return cudaGetLastError();

@@ -191,7 +191,11 @@ def test_topb_ties_nan_inf(B):
         check_exact(B.select_topb(shape, dev_f32(e)), oracle.topb(e, bk), f"top-B Bk={bk}")
 
 
-@pytest.mark.parametrize("C,Bk,chunks", [(512, 129, 64), (1024, 513, 16), (2047, 100, 8), (8191, 4000, 3), (5, 3, 200)])
+@pytest.mark.parametrize("C,Bk,chunks", [(512, 129, 64), (1024, 513, 16), (2047, 100, 8), (8191, 4000, 3), (5, 3, 200),
+                                           # the warp-per-chunk kernel's size classes (C <= 128 / 512 / 1024) and the first size beyond
+                                           # (taken from 1024 chunks on)
+                                           (128, 64, 1030), (129, 2, 1027), (512, 129, 1100), (513, 513, 1024), (1024, 1025, 1025),
+                                           (1024, 257, 1031), (1025, 300, 1024), (31, 32, 2000), (128, 64, 9), (513, 100, 1023)])
 def test_topb_random(B, C, Bk, chunks):
     r = np.random.default_rng(C + Bk)
     e = r.standard_normal((1, 1, chunks, C + 1)).astype(np.float32)
