@@ -23,6 +23,7 @@ namespace {
 
 constexpr int kTokThreads = 320;          // 8 softmax warps (two column halves) + TMA warp + MMA warp
 constexpr int kTokTmaWarp = 8, kTokMmaWarp = 9;
+constexpr int kTokTailGroup = 4;         // one-row tails (Cp = 128 t + 1) of this many consecutive chunks share a tile step (as in score.cu)
 
 struct TokParams {
     const uint16_t *Q;
@@ -59,10 +60,15 @@ token_score_kernel(const TokParams p, const __grid_constant__ CUtensorMap tmap12
     __shared__ uint32_t tmem_slot;
     __shared__ __align__(16) float s_l2[2][kTileM];      // -ell * log2(e) per scoring row of the tile (+inf beyond the rows)
     __shared__ float s_e1[2][kTileM];         // column half 1's partial sums, double-buffered by tile parity
+    __shared__ __align__(16) float s_l2t[kTokTailGroup][kTileM];   // -ell * log2(e) of a tail group's chunks (the shared tail step)
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int64_t u_lo = p.units * blockIdx.x / gridDim.x, u_hi = p.units * (blockIdx.x + 1) / gridDim.x;
     const int tiles_per_chunk = (p.Cp + kTileN - 1) / kTileN;
+    // chunks of 128 t + 1 rows: the one-row tails of kTokTailGroup consecutive chunks of a segment are taken in ONE tile step
+    // behind the main tiles of the group's first chunk (16-row TMA boxes side by side: chunk n + k's tail slot is tile row 16 k)
+    const bool tail_groups = tiles_per_chunk > 1 && p.Cp - (tiles_per_chunk - 1) * kTileN == 1;
+    const int main_tiles = tail_groups ? tiles_per_chunk - 1 : tiles_per_chunk;
 
     const uint32_t bar0 = smem_u32(&bars[0]);
     auto k_full = [&](int s) { return bar0 + 8u * s; };
@@ -115,11 +121,23 @@ token_score_kernel(const TokParams p, const __grid_constant__ CUtensorMap tmap12
             const uint64_t policy = l2_policy_evict_first();
             for (int n = n0; n < n1; ++n) {
                 const int64_t row0 = ((int64_t)bg * p.N + n) * p.Cp;
-                for (int tt = 0; tt < tiles_per_chunk; ++tt, ++q) {
+                const bool leader = tail_groups && (n - n0) % kTokTailGroup == 0;
+                for (int tt = 0; tt < main_tiles + (leader ? 1 : 0); ++tt, ++q) {
                     const int stage = q % ST;
                     const int valid = min(kTileN, p.Cp - tt * kTileN);
                     const bool small = valid <= 16;
                     mbar_wait(k_free(stage), ((q / ST) & 1) ^ 1);
+                    if (tt == main_tiles && tail_groups) {
+                        const int g = min(kTokTailGroup, n1 - n);
+                        mbar_arrive_expect_tx(k_full(stage), (uint32_t)(16 * g) * D * 2);
+                        for (int k = 0; k < g; ++k) {
+                            const int32_t trow = (int32_t)(row0 + (int64_t)k * p.Cp + (int64_t)main_tiles * kTileN);
+#pragma unroll
+                            for (int pn = 0; pn < Cfg::kPanels; ++pn)
+                                tma_load_2d(sK(stage) + pn * Cfg::kPanelBytes + (uint32_t)k * 2048u, &tmap16, pn * 64, trow, k_full(stage));
+                        }
+                        continue;
+                    }
                     mbar_arrive_expect_tx(k_full(stage), (uint32_t)(small ? 16 : 128) * D * 2);
                     const CUtensorMap *tm = small ? &tmap16 : &tmap128;
                     const int32_t row = (int32_t)(row0 + (int64_t)tt * kTileN);
@@ -140,7 +158,8 @@ token_score_kernel(const TokParams p, const __grid_constant__ CUtensorMap tmap12
         if (lane == 0) {
             constexpr uint32_t idesc = umma_idesc_bf16(kTileM, kTileN, 0, 0);
             for (int n = n0; n < n1; ++n) {
-                for (int tt = 0; tt < tiles_per_chunk; ++tt, ++q) {
+                const bool leader = tail_groups && (n - n0) % kTokTailGroup == 0;
+                for (int tt = 0; tt < main_tiles + (leader ? 1 : 0); ++tt, ++q) {
                     const int stage = q % ST, buf = q & 1;
                     mbar_wait(k_full(stage), (q / ST) & 1);
                     mbar_wait(s_free(buf), ((q >> 1) & 1) ^ 1);
@@ -168,17 +187,29 @@ token_score_kernel(const TokParams p, const __grid_constant__ CUtensorMap tmap12
             return m < p.rows ? -__ldg(p.row_lse + ((int64_t)bg * p.N + n) * p.rows + m) * kLog2e : -INFINITY;
         };
         float l2_next = tid < kTileM ? load_l2(n0) : 0.f;
+        float lt[kTokTailGroup];                       // the next tail group's values (threads 0..127), one group ahead
+#pragma unroll
+        for (int k = 0; k < kTokTailGroup; ++k) lt[k] = (tail_groups && tid < kTileM && n0 + k < n1) ? load_l2(n0 + k) : 0.f;
         float *e_out = p.e + (int64_t)mt * p.part_stride;
         for (int n = n0; n < n1; ++n) {
             const int par = (n - n0) & 1;
+            const bool leader = tail_groups && (n - n0) % kTokTailGroup == 0;
+            const int g = min(kTokTailGroup, n1 - n);      // chunks in the group this chunk leads
             if (tid < kTileM) {
                 s_l2[par][tid] = l2_next;
                 if (n + 1 < n1) l2_next = load_l2(n + 1);       // in flight under this chunk's tiles
+                if (leader) {
+#pragma unroll
+                    for (int k = 0; k < kTokTailGroup; ++k) {
+                        s_l2t[k][tid] = lt[k];
+                        if (n + kTokTailGroup + k < n1) lt[k] = load_l2(n + kTokTailGroup + k);
+                    }
+                }
             }
             asm volatile("bar.sync 1, 256;" ::: "memory");
             const float4 *l2v = reinterpret_cast<const float4 *>(&s_l2[par][64 * half]);
             // sum over 32 columns of 2^(c2*x - ell2[col]): packed f32x2 arithmetic, a quarter of the exponentials as polynomial
-            auto block_sum = [&](const uint32_t(&v)[32], int c0) {
+            auto block_sum = [&](const uint32_t(&v)[32], int c0, const float4 *l2v) {
                 const uint64_t c2v = pack_f32x2(p.c2, p.c2);
                 uint64_t acc0 = 0ull, acc1 = 0ull;
 #pragma unroll
@@ -201,9 +232,11 @@ token_score_kernel(const TokParams p, const __grid_constant__ CUtensorMap tmap12
                 unpack_f32x2(acc1, s2, s3);
                 return (s0 + s1) + (s2 + s3);
             };
-            for (int tt = 0; tt < tiles_per_chunk; ++tt, ++q) {
+            for (int tt = 0; tt < main_tiles + (leader ? 1 : 0); ++tt, ++q) {
                 const int buf = q & 1;
-                const int valid = min(kTileN, p.Cp - tt * kTileN);
+                const bool group_tail = tail_groups && tt == main_tiles;
+                // rows of the tile that are cache slots: a tile's first `valid` rows, or, in a group's tail step, rows 0, 16, ..
+                const int valid = group_tail ? 16 * (g - 1) + 1 : min(kTileN, p.Cp - tt * kTileN);
                 const uint32_t tS = tmem + 128u * buf + lane_base;
                 mbar_wait(s_ready(buf), (q >> 1) & 1);
                 tc_fence_after();
@@ -217,15 +250,24 @@ token_score_kernel(const TokParams p, const __grid_constant__ CUtensorMap tmap12
                 tmem_ld32(tS, va);
                 tmem_wait_ld();
                 tmem_ld32(tS + 32u, vb);
-                float sum = block_sum(va, 0);
+                // the subtrahends: this chunk's, or in a group's tail step those of the chunk whose tail this slot is
+                const int kk = group_tail ? min(row >> 4, g - 1) : 0;
+                const float4 *lv = group_tail ? reinterpret_cast<const float4 *>(&s_l2t[kk][64 * half]) : l2v;
+                float sum = block_sum(va, 0, lv);
                 tmem_wait_ld();
                 tc_fence_before();
                 mbar_arrive(s_free(buf));
-                sum += block_sum(vb, 32);
+                sum += block_sum(vb, 32, lv);
                 if (half == 1) s_e1[q & 1][row] = sum;
                 asm volatile("bar.sync %0, 64;" ::"r"(pair_bar) : "memory");
-                if (half == 0 && row < valid)
-                    e_out[((int64_t)bg * p.N + n) * p.Cp + tt * kTileN + row] = sum + s_e1[q & 1][row];
+                if (half == 0) {
+                    if (group_tail) {
+                        if ((row & 15) == 0 && (row >> 4) < g)
+                            e_out[((int64_t)bg * p.N + n + (row >> 4)) * p.Cp + tt * kTileN] = sum + s_e1[q & 1][row];
+                    } else if (row < valid) {
+                        e_out[((int64_t)bg * p.N + n) * p.Cp + tt * kTileN + row] = sum + s_e1[q & 1][row];
+                    }
+                }
             }
         }
     }

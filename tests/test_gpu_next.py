@@ -176,6 +176,24 @@ def test_token_scores_and_topb(B, name, kw):
     check_exact(keep, inp["keep"], "planted tokens (generator sanity)")
 
 
+@pytest.mark.parametrize("kw", [
+    dict(B=5, H=8, H_kv=8, d=64, N=512, C=128, K=4, L_q=16, L_d=8),     # Cp = 129: 69 chunks per CTA, runs cross (b, g) boundaries
+    dict(B=1, H=2, H_kv=2, d=128, N=301, C=128, K=3, L_q=128, L_d=8),   # 602 chunks / 296 CTAs: runs of 2-3, groups cut short
+    dict(B=1, H=6, H_kv=2, d=64, N=23, C=384, K=3, L_q=60, L_d=4),      # GQA G = 3: 180 rows = 2 M tiles (partials), Cp = 385
+    dict(B=1, H=4, H_kv=4, d=128, N=5, C=256, K=2, L_q=40, L_d=8),      # 20 chunks on 20 CTAs: every group a single chunk
+    dict(B=1, H=1, H_kv=1, d=128, N=1, C=1024, K=1, L_q=16, L_d=8),     # a single chunk
+    dict(B=5, H=8, H_kv=8, d=128, N=64, C=128, K=4, L_q=32, L_d=8),     # runs of 8-9 chunks = groups of 4, 4, (1)
+])
+def test_token_scores_one_row_tails_in_groups(B, kw):
+    """Chunks of 128 t + 1 rows: the token kernel takes the tail slots of up to four consecutive chunks of a CTA's run in
+    one tile step, each against its own chunk's row log-masses.  Every slot of every chunk against the oracle."""
+    w, inp = _inputs("tiny", **kw)
+    shape = B.Shape.of(w)
+    e = B.score_tokens(shape, dev_bf16(inp["Q_dec"]), dev_bf16(inp["Kcache"]))
+    torch.cuda.synchronize()
+    _check_e(e, oracle.token_scores(inp["Q_dec"], inp["Kcache"], w.L_q), w.G * w.L_q, "token scores (grouped tails)")
+
+
 def test_topb_ties_nan_inf(B):
     C, Bk = 40, 7
     e = np.zeros((1, 1, 7, C + 1), np.float32)
