@@ -356,11 +356,30 @@ def run_ours(args, w):
         K = K_save
         sustained = {"steps": max(200, K_save), "us_per_step": us_sus, "clocks": clk_s.summary()}
 
+    # ---- hot L2 (reported separately): workloads whose cache fits L2, stepped back to back WITHOUT the
+    # flush, so every call after the first finds K / V in L2.  Never `value`.
+    us_hot = us_attn_hot = None
+    if flush:
+        def hot_loop(fn):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            fn()
+            a.record()
+            for _ in range(K):
+                fn()
+            b.record()
+            barrier()
+            return 1e3 * a.elapsed_time(b) / K
+        barrier()
+        us_hot = hot_loop(step)
+
     # the paper's static-selection mode: per step only pdllm_sparse_attn
     ids = out["chunk_ids"].clone()
     barrier()
     us_attn_only = timed_loop(lambda: B.sparse_attn(shape, dQ, dKc, dVc, ids, dkeep, dKd, dVd, n_splits=args.n_splits,
                                                     O=out["O"], LSE=out["LSE"], workspace=ws))
+    if flush:
+        us_attn_hot = hot_loop(lambda: B.sparse_attn(shape, dQ, dKc, dVc, ids, dkeep, dKd, dVd, n_splits=args.n_splits,
+                                                     O=out["O"], LSE=out["LSE"], workspace=ws))
 
     # ---- e2e: HOST per-step tensors through pdllm_step_host, copies inside the timed region
     pin = lambda bits: torch.from_numpy(np.ascontiguousarray(bits).view(np.int16)).view(torch.bfloat16).pin_memory()
@@ -451,6 +470,7 @@ def run_ours(args, w):
             "stages_us": {"score_chunks": t_score, "select_topk": t_topk, "sparse_attn_partial": t_attn,
                           "lse_combine": t_comb, "step_with_stage_events": us_profiled,
                           "step_cuda_graph_replay": us_graph,
+                          "step_hot_l2_back_to_back": us_hot, "sparse_attn_only_hot_l2": us_attn_hot,
                           "sparse_attn_only_static_selection": us_attn_only},
             "sustained": sustained,
             "roofline": dominant, "roofline_attn": roof_attn, "roofline_score": roof_score,
