@@ -277,6 +277,8 @@ def run_ours(args, w):
     flush = needs_flush(w)
     flush_buf = torch.empty((256 << 20,), dtype=torch.uint8, device="cuda") if flush else None
 
+    per_call = []                         # flush mode: the last timed_loop's per-call times (median / min beside the mean)
+
     def timed_loop(fn):
         """us per call of fn over K calls: one event pair around the loop, or (flush mode) one pair per call with the
         L2 flush between calls outside the timed intervals."""
@@ -295,7 +297,9 @@ def run_ours(args, w):
             fn()
             b.record()
         barrier()
-        return 1e3 * sum(a.elapsed_time(b) for a, b in pairs) / K
+        per_call.clear()
+        per_call.extend(1e3 * a.elapsed_time(b) for a, b in pairs)
+        return sum(per_call) / K
 
     # ---- the timed regions, clocks sampled meanwhile: K steps through pdllm_step_profiled (per-stage CUDA events recorded
     # on the launching stream inside the loop: the stage split and the kernels' rooflines; the events cost a few us per
@@ -311,12 +315,15 @@ def run_ours(args, w):
         t_end.record()
         barrier()
         us_plain_rank = timed_loop(step)
+    plain_calls = sorted(per_call)        # empty without the flush: one event pair spans the whole loop there
     total_ms = max_over_ranks(us_plain_rank * K / 1e3, world)
     us_per_step = replica_us_per_step(total_ms, K, world)     # replicas: world independent steps ran per iteration
     if flush:
         us_profiled = 1e3 * sum(evs[k][0].elapsed_time(evs[k][4]) for k in range(K)) / K
     else:
         us_profiled = 1e3 * t_begin.elapsed_time(t_end) / K
+
+    staged_calls = sorted(1e3 * evs[k][0].elapsed_time(evs[k][4]) for k in range(K))
 
     def stage(i, j):
         return 1e3 * sum(evs[k][i].elapsed_time(evs[k][j]) for k in range(K)) / K
@@ -469,6 +476,8 @@ def run_ours(args, w):
                         "the rooflines come from K more steps through pdllm_step_profiled, run just before",
             "stages_us": {"score_chunks": t_score, "select_topk": t_topk, "sparse_attn_partial": t_attn,
                           "lse_combine": t_comb, "step_with_stage_events": us_profiled,
+                          "step_with_stage_events_median_min": [statistics.median(staged_calls), staged_calls[0]],
+                          "step_median_min": [statistics.median(plain_calls), plain_calls[0]] if plain_calls else None,
                           "step_cuda_graph_replay": us_graph,
                           "step_hot_l2_back_to_back": us_hot, "sparse_attn_only_hot_l2": us_attn_hot,
                           "sparse_attn_only_static_selection": us_attn_only},
