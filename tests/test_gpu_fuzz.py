@@ -108,3 +108,36 @@ def test_next_rows_random_shapes(seed):
         Op_ref, Lp_ref = oracle.prefill_attn(Qp, Kp, Vp)
         check_O(Op, Op_ref, what=f"prefill O ({what})")
         check_close(Lp, Lp_ref, LSE_ABS, what=f"prefill LSE ({what})")
+
+
+@pytest.mark.parametrize("kw,S", [
+    (dict(B=1, H=2, H_kv=2, d=64, N=4096, C=15, K=64, keep=1.0, L_q=16, L_d=16), 0),     # N and K at the header's bounds
+    (dict(B=1, H=4, H_kv=2, d=128, N=4096, C=7, K=33, keep=0.5, L_q=40, L_d=8), 2),      # 8-row chunks, thinned, GQA
+    (dict(B=1, H=2, H_kv=1, d=128, N=2, C=8191, K=2, keep=1.0, L_q=8, L_d=24), 0),       # the longest chunk top-B takes: 128 KV tiles
+    (dict(B=1, H=1, H_kv=1, d=64, N=3, C=8191, K=1, keep=0.37, L_q=130, L_d=0), 5),      # no decode block, two M tiles of scoring rows
+])
+def test_sizes_at_the_bounds(kw, S):
+    """The largest chunk count, selection size and chunk length the header allows, through the step and NEXT-1."""
+    from paper_2606_10537_b200 import binding as B
+    B.lib()
+    w = W.small_variant(W.CONFIGS["tiny"], **kw)
+    inp = W.make_inputs(w)
+    dev = to_device(inp)
+    shape = B.Shape.of(w)
+    out = B.step(shape, dev["Q_dec"], dev["Kcache"], dev["Vcache"], dev["keep"], dev["K_dec"], dev["V_dec"], n_splits=S)
+    torch.cuda.synchronize()
+    ref = oracle.step(inp["Q_dec"], inp["Kcache"], inp["Vcache"], inp["keep"], inp["K_dec"], inp["V_dec"], w.K, w.L_q)
+    check_close(out["scores"], ref["scores"], SCORE_ABS, what="scores")
+    ids = oracle.topk(out["scores"].double().cpu().numpy(), w.K)
+    check_exact(out["chunk_ids"], ids)
+    O_ref, LSE_ref = oracle.attn(inp["Q_dec"], inp["Kcache"], inp["Vcache"], ids, inp["keep"], inp["K_dec"], inp["V_dec"])
+    check_O(out["O"], O_ref)
+    check_close(out["LSE"], LSE_ref, LSE_ABS)
+    e = B.score_tokens(shape, dev["Q_dec"], dev["Kcache"])
+    torch.cuda.synchronize()
+    e_ref = oracle.token_scores(inp["Q_dec"], inp["Kcache"], w.L_q)
+    worst = float((np.abs(e.double().cpu().numpy() - e_ref) - (1e-4 * np.abs(e_ref) + 1e-6 * w.G * w.L_q)).max())
+    assert worst <= 0, f"token scores gate exceeded by {worst:.3e}"
+    keep = B.select_topb(shape, e)
+    torch.cuda.synchronize()
+    check_exact(keep, oracle.topb(e.double().cpu().numpy(), w.Bk), "top-B")
