@@ -98,8 +98,9 @@ const char *pdllm_strerror(int status);        /* static string, never NULL */
  * for num_sms SMs (<= 0: the current device's count).  Per candidate S in
  * 1..min(KV tiles, 64) the model takes the busiest CTA's KV-tile steps under the
  * kernel's item order (plus a fixed cost per work item) and, for S > 1, the
- * combine step's launch and its 2*S*rows*d*4 bytes of partial traffic; the
- * cheapest S wins, a larger S only by a 3 % margin.  A split may be a single
+ * combine step's launch and its 2*S*rows*d*4 bytes of partial traffic (at L2
+ * speed while they fit L2, at HBM speed beyond); the constants are fitted to
+ * measured split sweeps; the cheapest S wins, a larger S only by a 3 % margin.  A split may be a single
  * 128-row KV tile; never more splits than KV tiles.  >= 1. */
 int32_t pdllm_auto_splits(const pdllm_shape *shape, int32_t num_sms);
 

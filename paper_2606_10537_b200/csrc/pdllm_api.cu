@@ -63,7 +63,10 @@ int resolve(const pdllm_shape *sh, bool has_keep, Dims *out) {
 double split_cost_us(const Dims &d, int S, int sms) {
     const int T = kv_tiles(d), BG = d.B * d.H_kv;
     const int n_qt = (d.rows_g + kTileM - 1) / kTileM, n_pairs = n_qt / 2, n_single = n_qt & 1;
-    const double kStepUs = 1.3, kItemSteps = 1.5, kLaunchUs = 3.0, kHbmBytesPerUs = 6.0e6;
+    // constants fitted to the measured split sweeps (profiles/r2_splitsweep_dream16k.md, C2-C4, the Fig. 5(b) shapes) and checked
+    // on the configs[4] sweep: partials that stay in L2 (write + read <= 64 MB) move at ~8 TB/s, larger ones through HBM
+    // against the attention's own traffic at ~3 TB/s
+    const double kStepUs = 1.3, kItemSteps = 0.5, kLaunchUs = 1.0, kL2BytesPerUs = 8.0e6, kHbmBytesPerUs = 3.0e6, kL2Traffic = 64.0e6;
     const int64_t na = (int64_t)BG * n_pairs * S, nb = (int64_t)BG * n_single * S;
     const double ca = (T + S - 1) / S + kItemSteps, cb = ((T + S - 1) / S + 1) / 2 + kItemSteps;
     // CTA c receives items c, c + sms, ...: those below na cost ca, the rest cb
@@ -75,7 +78,10 @@ double split_cost_us(const Dims &d, int S, int sms) {
         if (load > worst) worst = load;
     }
     double us = worst * kStepUs;
-    if (S > 1) us += kLaunchUs + 2.0 * S * (double)d.B * d.H * d.L * d.d * 4.0 / kHbmBytesPerUs;
+    if (S > 1) {
+        const double traffic = 2.0 * S * (double)d.B * d.H * d.L * d.d * 4.0;
+        us += kLaunchUs + traffic / (traffic <= kL2Traffic ? kL2BytesPerUs : kHbmBytesPerUs);
+    }
     return us;
 }
 
