@@ -19,6 +19,7 @@ __global__ void __launch_bounds__(kCombineWarps * 32) combine_kernel(const float
     // launched as a programmatic dependent of the kernel that writes the partials (its launch is processed while that
     // kernel still runs): wait for that grid's completion and flush before reading them
     asm volatile("griddepcontrol.wait;" ::: "memory");
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");      // (the next step's score kernel)
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int64_t row = (int64_t)blockIdx.x * kCombineWarps + warp;
     if (row >= rows) return;

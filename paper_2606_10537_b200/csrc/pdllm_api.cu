@@ -489,14 +489,13 @@ int pdllm_step_profiled(const pdllm_shape *shape, const void *Q_dec, const void 
     if (!aligned16(scores_out)) return PDLLM_ERR_ALIGN;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     if (int rc = debug_validate(d, nullptr, token_keep_idx, st)) return rc;
-    // the attention's work-item counter is cleared here, far ahead of its kernel (off the step's critical path)
-    if (int rc = cuda_rc(cudaMemsetAsync(workspace, 0, sizeof(int32_t), st))) return rc;
+    // the attention's work-item counter is cleared by the score kernel (no memset node between the step's kernels)
     if (int rc = record(ev ? ev->begin : nullptr, st)) return rc;
     // with several M tiles of scoring rows (G*L_q > 128) the score kernel leaves per-M-tile partials in the workspace
     // and the top-K kernel sums them in M-tile order: no float atomics, bit-reproducible scores
     float *sp = score_partial_bytes(d) ? reinterpret_cast<float *>(static_cast<char *>(workspace) + kCounterBytes + partials_bytes(d, S))
                                        : nullptr;
-    if (int rc = cuda_rc(launch_score(d, Q_dec, (int64_t)d.H * d.L * d.d, (int64_t)d.L * d.d, Kcache, scores_out, nullptr, sp, st)))
+    if (int rc = cuda_rc(launch_score(d, Q_dec, (int64_t)d.H * d.L * d.d, (int64_t)d.L * d.d, Kcache, scores_out, nullptr, sp, st, static_cast<int32_t *>(workspace))))
         return rc;
     // a2 inside the attention kernel (one launch fewer; the attention becomes the score kernel's programmatic
     // dependent) when the chunk count allows it, no gather-index export wants the ids ahead of a4 and no stage
@@ -562,9 +561,8 @@ int pdllm_step_host(const pdllm_shape *shape, const void *h_Q_dec, const void *h
     if (cudaMemcpyAsync(base + h.kd, h_K_dec, kb, cudaMemcpyHostToDevice, st2) != cudaSuccess) return PDLLM_ERR_CUDA;
     if (cudaMemcpyAsync(base + h.vd, h_V_dec, kb, cudaMemcpyHostToDevice, st2) != cudaSuccess) return PDLLM_ERR_CUDA;
     if (side && cudaEventRecord(ev_join, st2) != cudaSuccess) return PDLLM_ERR_CUDA;
-    if (int rc = cuda_rc(cudaMemsetAsync(base + h.ws, 0, sizeof(int32_t), st))) return rc;
     float *sp = score_partial_bytes(dv) ? reinterpret_cast<float *>(base + h.ws + kCounterBytes + partials_bytes(dv, Sv)) : nullptr;
-    if (int rc = cuda_rc(launch_score(dv, base + h.q, (int64_t)dv.H * dv.L * dv.d, (int64_t)dv.L * dv.d, d_Kcache, scores, nullptr, sp, st)))
+    if (int rc = cuda_rc(launch_score(dv, base + h.q, (int64_t)dv.H * dv.L * dv.d, (int64_t)dv.L * dv.d, d_Kcache, scores, nullptr, sp, st, reinterpret_cast<int32_t *>(base + h.ws))))
         return rc;
     const bool fold_topk = attn_can_fold_topk(dv) && !no_fold();
     if (!fold_topk)

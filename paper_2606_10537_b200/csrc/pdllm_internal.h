@@ -39,7 +39,7 @@ cudaError_t launch_combine(const float *O_part, const float *lse_part, int S, in
 // ---- a1: scores[b,g,n]
 // row_lse (optional): [B*H_kv, N, G*L_q] fp32, every scoring row's log-mass per chunk
 cudaError_t launch_score(const Dims &s, const void *Q, int64_t q_batch_stride, int64_t q_head_stride, const void *Kcache,
-                         float *scores, float *row_lse, float *partials, cudaStream_t st);
+                         float *scores, float *row_lse, float *partials, cudaStream_t st, int32_t *zero_counter = nullptr);
 // ---- NEXT-1 (token_score.cu): e [B,H_kv,N,Cp] from row_lse; e_part: [m_tiles, B,H_kv,N,Cp] scratch when G*L_q > 128
 cudaError_t launch_token_scores(const Dims &s, const void *Q, int64_t q_batch_stride, int64_t q_head_stride,
                                 const void *Kcache, const float *row_lse, float *e, float *e_part, cudaStream_t st);

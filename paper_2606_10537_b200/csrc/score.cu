@@ -37,6 +37,7 @@ struct ScoreParams {
     float c2, inv_rows;
     int use_atomic, evict_first;          // use_atomic: several M tiles add into scores[] (order not fixed)
     float *partials;                      // or, when given: [m_tiles, B*H_kv*N] plain stores, summed in M-tile order by the consumer
+    int32_t *zero_counter;                // pdllm_step: the attention kernel's work-item counters, cleared here (no memset node)
 };
 
 template <int D>
@@ -102,6 +103,14 @@ score_kernel(const ScoreParams p, const __grid_constant__ CUtensorMap tmap128, c
     tc_fence_after();
     const uint32_t tmem = tmem_slot;
     int q = 0;                                // tile-step counter of the K ring / S buffers (every role counts alike)
+    // The kernel is itself launched as a programmatic dependent of whatever precedes it in the stream (in a denoising loop:
+    // the previous step's attention / combine kernel): the set-up above ran under that kernel's tail; nothing it may have
+    // written (Q, the cache, the counters) is touched before this wait.
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    if (p.zero_counter && blockIdx.x == 0 && tid == 0) {
+        p.zero_counter[0] = 0;                // the attention kernel reads them behind its own wait on this grid
+        p.zero_counter[1] = 0;
+    }
 
     for (int64_t u = u_lo; u < u_hi;) {
     // ---- one segment: up to kMaxChunksPerCta consecutive chunks n0..n1-1 of one (bg, M tile)
@@ -423,16 +432,25 @@ cudaError_t launch_score_d(const ScoreParams &p, const CUtensorMap &t128, const 
     cudaError_t e = cudaFuncSetAttribute(score_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::kSmem);
     if (e != cudaSuccess) return e;
     const int64_t slots = 2ll * device_num_sms();          // two CTAs per SM
-    dim3 grid((unsigned)(p.units < slots ? p.units : slots), 1, 1);
-    score_kernel<D><<<grid, kScoreThreads, Cfg::kSmem, st>>>(p, t128, t16);
-    return cudaGetLastError();
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)(p.units < slots ? p.units : slots), 1, 1);
+    cfg.blockDim = dim3(kScoreThreads, 1, 1);
+    cfg.dynamicSmemBytes = Cfg::kSmem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, score_kernel<D>, p, t128, t16);
 }
 
 }  // namespace
 
 cudaError_t launch_score(const Dims &s, const void *Q, int64_t q_batch_stride, int64_t q_head_stride, const void *Kcache,
-                         float *scores, float *row_lse, float *partials, cudaStream_t st) {
+                         float *scores, float *row_lse, float *partials, cudaStream_t st, int32_t *zero_counter) {
     ScoreParams p;
+    p.zero_counter = zero_counter;
     p.Q = static_cast<const uint16_t *>(Q);
     p.q_batch_stride = q_batch_stride;
     p.q_head_stride = q_head_stride;
