@@ -39,6 +39,12 @@
  *     (this mode allocates and frees a 4-byte device flag per call: the one
  *     exception to the rules above; for pdllm_step* the ids are produced
  *     internally, so only the keep list is checked).
+ *   - STREAM ORDER: the kernels are launched with programmatic stream
+ *     serialisation: a kernel's set-up may run under the tail of the kernel before
+ *     it in the stream (yours included), but it touches no global memory before
+ *     that kernel has completed and its writes are visible
+ *     (griddepcontrol.wait), so the usual in-stream ordering holds for every
+ *     buffer you pass.
  *   - bf16 = IEEE bfloat16 bit patterns; O is rounded to bf16 round-to-nearest-even
  *     from the fp32 accumulator (R11).
  *   - GQA: query head h reads KV head h / (H / H_kv) (R4).
