@@ -47,6 +47,17 @@ def test_auto_splits(name, expect_min, expect_max):
     assert expect_min <= s <= expect_max, s
 
 
+@pytest.mark.parametrize("name", ["fig5b", "fig5b_8k", "fig5b_16k", "fig5b_32k"])
+def test_auto_splits_fig5b_shapes_fill_one_wave(name):
+    """The Fig. 5(b) decode shapes are 8 KV groups of one query tile: the split count is what turns them into about one
+    wave of work items (8 * S <= 148 SMs), far beyond the paper's S = 4 (measured: profiles/r2_splitsweep_dream16k.md)."""
+    s = B.auto_splits(B.Shape.of(W.EXTRA[name]), 148)
+    assert 11 <= s <= 18, s
+    # a big batch needs none: its work items fill the SMs by themselves and its partials would go through HBM
+    big = W.small_variant(W.CONFIGS["sparse32k"], B=8, N=16, C=1024, K=16, keep=1.0, L_q=64, L_d=512)
+    assert B.auto_splits(B.Shape.of(big), 148) == 1
+
+
 def test_workspace_bytes():
     w = W.CONFIGS["sparse32k"]
     sh = B.Shape.of(w)
